@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the StePS cylindrical hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--n 1048576] [--precision fp64|mixed] [--n-cut 5]
+
+A "step" is one KDK leapfrog step of Eq. 11 over the whole particle set: background term,
+kick + drift, pack + wrap, the all-pairs image sum (Eq. 8), reduction, background term, kick --
+i.e. every row of the hot-path table, one force evaluation per step.  The workload is
+BASELINE.json configs[3] (N = 1 048 576, LCDM comoving load, L = 100 Mpc/h, n_cut = 5), the
+configuration the metric "pair interactions/s (N=1M, periodic-z, fp64)" is quoted on.
+
+Prints ONE JSON line.  `value` = ordered pairs N(N-1) per second of whole-step time, inputs
+resident in HBM.  `e2e` = the same through steps_cyl_kdk_step_host with pinned HOST buffers
+(host->device and device->host copies inside the timed region).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# FP64-pipe instruction mix of pair_fp64_kernel<5,0>, one (i, j) pair = 10 image terms, counted in
+# the SASS of the shipped kernel: 49 DFMA + 33 DMUL + 24 DADD + 3 DSETP.
+FP64_MIX = {5: dict(dfma=49, dmul=33, dadd=24, dsetp=3)}
+METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
+NOMINAL_FP64_LANES_PER_SM = 64
+
+
+def pipe_counts(n_cut):
+    """(FP64-pipe instructions, flops) per ordered pair; n_cut != 5 scales the per-image part."""
+    mix = FP64_MIX[5]
+    instr5 = sum(mix.values())
+    flops5 = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
+    if n_cut == 5:
+        return instr5, flops5
+    per_img_i, per_img_f = 9.5, 14.0                     # far image: 9.5 instr (5 FMA) / 14 flops
+    d = 2 * (n_cut - 5)
+    return instr5 + per_img_i * d, flops5 + per_img_f * d
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="steps_clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)),
+                       power_w_max=float(max(pw)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def cosmo_schedule(w, n_steps_total):
+    """(a_n, H_n, a_np1, H_np1) for consecutive KDK steps, from the library's own RK4."""
+    from paper_2602_20787_b200 import binding as b
+    c = w.cosmo
+    a = c["a_init"]
+    _, H = b.friedmann_step(a, 0.0, c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+    sched = []
+    for _ in range(n_steps_total):
+        a1, H1 = b.friedmann_step(a, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+        sched.append((a, H, a1, H1))
+        a, H = a1, H1
+    return sched
+
+
+def oracle_sample(w, seconds, n_cut):
+    """Time the oracle, as it stands, on a bounded seeded sample of targets x all N sources."""
+    import oracle
+    from paper_2602_20787_b200 import workloads
+    oracle.build()
+    cores = oracle.max_threads()
+    probe = workloads.sample_targets(w.n, 2 * cores, seed=99)
+    t0 = time.perf_counter()
+    oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, n_cut, targets=probe)
+    per_target = (time.perf_counter() - t0) / len(probe)
+    T = int(max(cores, min(w.n, seconds / max(per_target, 1e-9))))
+    T -= T % cores or 0
+    T = max(T, cores)
+    idx = workloads.sample_targets(w.n, T, seed=100)
+    return idx, cores
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same workload / metric / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(3, n=args.n)
+    idx, cores = oracle_sample(w, args.ref_seconds, args.n_cut)
+    times = []
+    for s in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, args.n_cut, targets=idx)
+        dt = time.perf_counter() - t0
+        if s >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    value = len(idx) * (w.n - 1) / t
+    sample = ("oracle.accel (force evaluation only) on %d seeded targets x all %d sources per step, "
+              "n_cut=%d" % (len(idx), w.n, args.n_cut))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "pairs/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving load, L=100, n_cut=%d, "
+                               "bounded target sample" % (w.n, args.n_cut)},
+        "image_terms_per_s": value * 2 * args.n_cut,
+        "cpu_baseline": {"value": value, "unit": "pairs/s", "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import build, workloads
+    build.build()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    prec = b.PREC_MIXED if args.precision == "mixed" else b.PREC_FP64
+    # replicas only: every rank integrates its own particle set
+    w = workloads.make(3, n=args.n, seed=3 + rank)
+    n = w.n
+    ctx = b.StepsCyl(n=n, Lz=w.Lz, G=w.G, n_cut=args.n_cut, precision=prec, background=b.BG_FINITE,
+                     R_sim=w.R_sim, rho0=w.rho0, device=local)
+    names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
+    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
+            for k in names}
+    dev = {k: host[k].cuda(non_blocking=True) for k in names}
+    g = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)       # g(x_0), untimed
+    ctx.check()
+    hg = [t.cpu().pin_memory() for t in g]
+    dfma_per_s = ctx.fp64_peak(200.0)
+    sched = cosmo_schedule(w, 2 * (args.warmup + args.steps) + 2)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def step(k):
+        flush.zero_()
+        ctx.kdk_step(*[dev[q] for q in names], *g, *sched[k], w.cosmo["dt"])
+
+    launches0 = ctx.launch_count()
+    for k in range(args.warmup):
+        step(k)
+    launches_per_step = (ctx.launch_count() - launches0) / max(args.warmup, 1)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    pair_ms = []
+    ev[0].record()
+    for k in range(args.steps):
+        step(args.warmup + k)
+        pair_ms.append(ctx.last_pair_kernel_ms())          # waits for that launch's end event
+    ev[1].record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else {}
+    ctx.check()
+    ms = torch.tensor([ev[0].elapsed_time(ev[1])], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    t_dev = float(ms.item()) * 1e-3
+    pairs_per_step = float(n) * float(n - 1)
+    value = world * pairs_per_step * args.steps / t_dev
+
+    # end to end: pinned host buffers through steps_cyl_kdk_step_host, copies inside the timing
+    hs = [host[q] for q in names] + hg
+    for k in range(1):
+        ctx.kdk_step_host(*hs, *sched[args.warmup + args.steps + k], w.cosmo["dt"])
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        ctx.kdk_step_host(*hs, *sched[args.warmup + args.steps + 1 + k], w.cosmo["dt"])
+    torch.cuda.synchronize()
+    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * pairs_per_step * args.steps / float(te.item())
+    assert all(bool(torch.isfinite(t).all()) for t in hg)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peaks, peaks_kind = load_peaks()
+    instr, flops = pipe_counts(args.n_cut)
+    t_pair = float(np.mean(pair_ms)) * 1e-3
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    nominal_tflops = sm_count * NOMINAL_FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    achieved_tflops = flops * pairs_per_step / t_pair / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "pair_%s_kernel<%d>" % (args.precision, args.n_cut),
+        "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
+        "frac": achieved_tflops / nominal_tflops, "traffic": None,
+        "peak_kind": "nominal FP64 FMA: %d SMs x 64 lanes x 2 flop x %.0f MHz (DESIGN.md)" % (sm_count, sm_max),
+        "flops_per_pair": flops, "fp64_pipe_instr_per_pair": instr,
+        "measured_dfma_tflops": 2 * dfma_per_s / 1e12,
+        "fp64_pipe_util_vs_measured_dfma": instr * pairs_per_step / t_pair / dfma_per_s,
+        "fp64_pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
+        "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
+    }
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        idx, cores = oracle_sample(w, args.ref_seconds, args.n_cut)
+        t0 = time.perf_counter()
+        oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, args.n_cut, targets=idx)
+        tc = time.perf_counter() - t0
+        cpu = {"value": len(idx) * (n - 1) / tc, "unit": "pairs/s", "cores": cores, "kind": "oracle",
+               "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
+                         "%.1f s" % (len(idx), n, tc)}
+    line = {
+        "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if prec == b.PREC_FP64 else "f32 pair terms / f64 accumulate",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving KDK step (Om=0.3, OL=0.7, "
+                               "a 0.02->0.025), L=100 Mpc/h, r_max=1000, n_cut=%d (10 images/pair), "
+                               "background Eq. 9" % (n, args.n_cut),
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "256 MiB buffer written between steps (L2 flush)"},
+        "image_terms_per_s": value * 2 * args.n_cut,
+        "seconds_per_force_evaluation": t_pair,
+        "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": 11 * 8 * n,
+                "d2h_bytes_per_step": 9 * 8 * n},
+        "gpu_launches": int(round(launches_per_step * args.steps)),
+        "peaks_file": peaks_kind,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=1048576)
+    ap.add_argument("--n-cut", type=int, default=5)
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"])
+    ap.add_argument("--ref-seconds", type=float, default=12.0,
+                    help="CPU seconds of oracle work per sample / reference step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

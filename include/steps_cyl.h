@@ -1,0 +1,182 @@
+/*
+ * steps_cyl.h -- C ABI of libsteps_cyl.so: the data-parallel hot path of the StePS
+ * cylindrical (S^1 x R^2, periodic along z, open in x-y) N-body method of
+ * arXiv 2602.20787 ("PAPER.md" below = /root/reference/PAPER.md), on one NVIDIA B200
+ * (sm_100a).
+ *
+ * What the library computes
+ *   steps_cyl_accel    g_i = sum_{j != i} m_j F_{S1xR2}(x_i - x_j, h_i + h_j)
+ *                      Eq. 1 with the one-axis-periodic pair law of Eq. 8
+ *                      (PAPER.md:85-90): the truncated z-image sum of the R^3 law Eq. 4
+ *                       through the cubic-spline softening Eq. 3
+ *                      (PAPER.md:56-61).  g includes G; it EXCLUDES 1/a^3, the Hubble drag
+ *                      and the background term of Eq. 11 -- those are applied in kdk_step.
+ *   steps_cyl_background
+ *                      b_i = -F_h(rho_i; R_sim, N_cut L_z) e_rho: the homogeneous-cylinder
+ *                      term of Eq. 11, F_h from Eq. 9 or
+ *                      its N_cut -> infinity limit Eq. 10.
+ *   steps_cyl_kdk_step one kick-drift-kick leapfrog step of Eq. 11 in cosmic time t
+ *                      (PAPER.md:128-133), comoving coordinates.
+ *   steps_cyl_friedmann_step
+ *                      one RK4 step of the Friedmann equation Eq. 18,
+ *                      host scalars.
+ *
+ * Conventions common to all calls
+ *   - Every function returns STEPS_OK (0) or a negative steps_cyl_status.  Nothing throws,
+ *     aborts or prints.  steps_cyl_strerror(code) gives a static string; for STEPS_ECUDA the
+ *     text of the last CUDA error seen by that context is available through
+ *     steps_cyl_last_cuda_error(ctx).
+ *   - "device pointer" = CUDA global memory on params.device; "host pointer" = ordinary (or
+ *     pinned) host memory.  All arrays are contiguous double precision, length n, SoA (one
+ *     array per coordinate).  The caller owns every particle array; the context owns only its
+ *     scratch and tables.  No pointer is retained after a call returns.
+ *   - Device-pointer calls are ASYNCHRONOUS: work is enqueued on `cuda_stream` (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream) and the call returns without
+ *     synchronising.  Host-pointer calls (…_host) copy in, compute, copy out and synchronise
+ *     the context's own stream before returning.
+ *   - One context serves one stream at a time: calls on one context must be serialised by the
+ *     caller.  Different contexts are independent.
+ *   - z may lie outside [0, Lz): it is reduced to [0, Lz) first (periodicity).
+ *     NaN / Inf inputs are not checked (garbage in, garbage out).
+ *   - There is NO CPU fallback: without a CUDA device steps_cyl_init returns STEPS_ECUDA.
+ */
+#ifndef STEPS_CYL_H
+#define STEPS_CYL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    STEPS_OK           =  0,
+    STEPS_EINVAL       = -1,  /* bad argument: n < 1, Lz <= 0, n_cut < 1, NULL pointer, unknown enum   */
+    STEPS_ESOFT        = -2,  /* softening precondition violated: some h_i <= 0 (or NaN)                   */
+    STEPS_ECUDA        = -3,  /* a CUDA runtime call failed (or no device present)                     */
+    STEPS_ENOMEM       = -4,  /* host or device allocation failed                                      */
+    STEPS_EUNSUPPORTED = -5   /* a mode that this build does not contain (EWALD_TABLE)                 */
+} steps_cyl_status;
+
+enum { STEPS_PERIODIC_IMAGES = 0,      /* Eq. 8, truncated image sum                                  */
+       STEPS_PERIODIC_EWALD_TABLE = 1  /* Eq. 12-17, lookup-table correction: not built yet            */ };
+enum { STEPS_PREC_FP64 = 0,            /* every pair term and the accumulation in double               */
+       STEPS_PREC_MIXED = 1            /* pair terms in float (cancellation-safe separations),
+                                          accumulation over sources in double                          */ };
+enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz                                    */
+       STEPS_BG_INFINITE = 1           /* Eq. 10                                                       */ };
+
+typedef struct steps_cyl_ctx steps_cyl_ctx;   /* opaque; created by init, freed by destroy */
+
+/* Plain-old-data parameter block (the quantities the problem statement
+ * names).  Zero-initialise, then fill. */
+typedef struct {
+    int64_t n;              /* number of particles, 1 <= n < 2^31                                     */
+    double  Lz;             /* period along z, > 0                                      */
+    double  G;              /* gravitational constant, any sign (G < 0: glass making)   */
+    int32_t periodic_mode;  /* STEPS_PERIODIC_*                                                       */
+    int32_t n_cut;          /* N_cut of Eq. 8, >= 1: 2*N_cut images per pair                          */
+    int32_t precision;      /* STEPS_PREC_*                                                           */
+    int32_t background;     /* STEPS_BG_*                                                             */
+    double  R_sim;          /* radius R of the simulation volume in Eq. 9; needed if rho0 != 0 and
+                               background == STEPS_BG_FINITE                                          */
+    double  rho0;           /* comoving mean density of Eq. 9/10; 0 disables the background term      */
+    int32_t device;         /* CUDA device ordinal                                                    */
+    int32_t reserved;       /* must be 0                                                              */
+} steps_cyl_params;
+
+/* Validate `p`, select the device, allocate scratch for n particles and build the constant
+ * tables (image offsets, quadrature nodes of Eq. 9).  Host-synchronous.
+ * Errors: EINVAL, EUNSUPPORTED (periodic_mode == EWALD_TABLE), ECUDA, ENOMEM. */
+int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out);
+
+/* Free everything the context owns.  NULL is allowed. */
+void steps_cyl_destroy(steps_cyl_ctx *ctx);
+
+/* g_i = sum_{j != i} m_j F_{S1xR2}(x_i - x_j, h_i + h_j)            (Eq. 1 + Eq. 8 + Eq. 3/4)
+ * in : x y z m h   device pointers, length n, read only
+ * out: gx gy gz    device pointers, length n, overwritten
+ * Asynchronous on cuda_stream.  The softening precondition (every h_i > 0) is checked on the
+ * device; its violation is reported by the next call to steps_cyl_check(ctx, stream) (which
+ * synchronises), and the outputs are then unspecified.  When 2*max(h) <= Lz/2 only the nearest
+ * image of a pair can lie inside the spline support and the fast kernel runs; otherwise
+ * (reading S7) a general kernel sends every image through Eq. 3 -- same result, slower; the
+ * choice is made on the device, with no host synchronisation. */
+int steps_cyl_accel(steps_cyl_ctx *ctx,
+                    const double *x, const double *y, const double *z,
+                    const double *m, const double *h,
+                    double *gx, double *gy, double *gz, void *cuda_stream);
+
+/* Same, with HOST pointers: copies the five inputs to the device, runs the same kernels,
+ * copies the three outputs back, synchronises, and reports ESOFT directly. */
+int steps_cyl_accel_host(steps_cyl_ctx *ctx,
+                         const double *x, const double *y, const double *z,
+                         const double *m, const double *h,
+                         double *gx, double *gy, double *gz);
+
+/* Synchronise `cuda_stream` and return the deferred status of the calls enqueued so far on
+ * this context (STEPS_OK, STEPS_ESOFT or STEPS_ECUDA); clears it. */
+int steps_cyl_check(steps_cyl_ctx *ctx, void *cuda_stream);
+
+/* b_i = -F_h(rho_i) (x_i, y_i)/rho_i, rho_i = sqrt(x_i^2 + y_i^2)   (Eq. 9 / Eq. 10, Eq. 11)
+ * in : x y   device pointers, length n;   out: bx by  device pointers, length n.
+ * rho0 == 0 writes zeros.  Asynchronous on cuda_stream. */
+int steps_cyl_background(steps_cyl_ctx *ctx, const double *x, const double *y,
+                         double *bx, double *by, void *cuda_stream);
+
+/* One KDK leapfrog step of Eq. 11 in cosmic time (readings S4, G5):
+ *   kick1 : v <- v + (dt/2) [ (g + b)/a_n^3 - 2 H_n v ]
+ *   drift : x <- x + v dt ;  z reduced to [0, Lz)
+ *   force : g <- steps_cyl_accel(x) ;  b <- steps_cyl_background(x)
+ *   kick2 : v <- [ v + (dt/2) (g + b)/a_np1^3 ] / (1 + H_np1 dt)
+ * in/out: x y z vx vy vz   device pointers, length n, updated in place
+ * in    : m h              device pointers, length n
+ * in/out: gx gy gz         on entry g(x_n) (from steps_cyl_accel or the previous step), on
+ *                          return g(x_{n+1})
+ * a_n, H_n, a_np1, H_np1   scale factor and Hubble parameter at t_n and t_n + dt (from the
+ *                          caller, e.g. steps_cyl_friedmann_step); dt the step in cosmic time.
+ * Asynchronous on cuda_stream. */
+int steps_cyl_kdk_step(steps_cyl_ctx *ctx,
+                       double *x, double *y, double *z,
+                       double *vx, double *vy, double *vz,
+                       const double *m, const double *h,
+                       double *gx, double *gy, double *gz,
+                       double a_n, double H_n, double a_np1, double H_np1, double dt,
+                       void *cuda_stream);
+
+/* Same step with HOST pointers: copies the eleven arrays to the device (88 B/particle), runs the
+ * same kernels, copies x y z vx vy vz gx gy gz back (72 B/particle), synchronises, and reports
+ * ESOFT directly.  This is the end-to-end form bench.py times. */
+int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx,
+                            double *x, double *y, double *z,
+                            double *vx, double *vy, double *vz,
+                            const double *m, const double *h,
+                            double *gx, double *gy, double *gz,
+                            double a_n, double H_n, double a_np1, double H_np1, double dt);
+
+/* Friedmann equation Eq. 18 with a cosmological constant:
+ * H(a) = H0 sqrt(Or a^-4 + Om a^-3 + Ok a^-2 + OL); one classical RK4 step of da/dt = a H(a)
+ * with the N-body step dt.  Host only, no context.  EINVAL on NULL / a <= 0. */
+int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double Or, double Ok,
+                             double OL, double *a_next, double *H_next);
+
+/* Measured ceiling of the FP64 pipe: runs an unrolled chain of independent DFMAs on every SM
+ * of the context's device for about `ms` milliseconds and returns DFMA instructions per
+ * second (thread-level) in *dfma_per_s.  Used by bench.py for the roofline denominator.
+ * Host-synchronous. */
+int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s);
+
+/* Milliseconds the device spent in the most recent all-pairs kernel launch of this context
+ * (CUDA events recorded around that launch on its stream); synchronises on the end event. */
+int steps_cyl_last_pair_kernel_ms(steps_cyl_ctx *ctx, float *ms);
+
+const char *steps_cyl_strerror(int code);
+const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx);
+
+/* Number of kernels this context has launched since init (bench.py's gpu_launches). */
+int64_t steps_cyl_launch_count(steps_cyl_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STEPS_CYL_H */

@@ -1,0 +1,226 @@
+// pair_fp64.cuh -- all-pairs S^1 x R^2 acceleration, every pair term in double precision.
+//
+// Computes, for each target i, the four partial sums over a chunk of sources j
+//     A_x  = sum_j m_j S_ij r_x,   A_y = sum_j m_j S_ij r_y,
+//     A_z1 = sum_j m_j S_ij r_z,   A_z2 = sum_j m_j T_ij,
+// where r = x_i - x_j with r_z reduced to the nearest image, and over the image set of
+// Eq. 8 (readings G2/S1)
+//     S_ij = sum_n w_n,   T_ij = sum_n n w_n,   w_n = F(s_n, h_i + h_j)/s_n,
+//     s_n^2 = rho^2 + (r_z - n L)^2,
+// F the spline of Eq. 3 (reading G1).  Because sum_n w_n (r_z - n L) =
+// r_z S - L T, the acceleration of Eq. 1/4/8 is g = -G (A_x, A_y, A_z1 - L A_z2); that last
+// step is done by finalize_kernel (aux_kernels.cuh).
+//
+// FP64-pipe bound: the design goal is the fewest FP64-pipe instructions per image term.
+//   * images +n and -n share B_n = q + n^2 L^2 (q = rho^2 + r_z^2):
+//         s_{+-n}^2 = fma(-+2 n L, r_z, B_n)                       3 instr / 2 images
+//   * w = (s^2)^(-3/2) from MUFU.RSQ64H (XU pipe, 20-bit seed y0, low word zero so y0^2 is
+//     exact) and one third-order step:  e = 1 - s^2 y0^2,  w = y0^3 (1 + 3e/2 + 15e^2/8)
+//                                                                    6 instr / image
+//   * S += w, T += n (w_+ - w_-)                                     2 instr / image
+//   * the spline can only act on the nearest image when 2 max(h) <= L/2 (checked on the
+//     device); it is a divergent slow path taken only by warps with a pair inside the support.
+// Sources are staged per CTA in shared memory and read as warp-wide broadcasts.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace steps {
+
+constexpr int PAIR_THREADS = 128;   // targets per CTA (one per thread) == sources per tile
+constexpr int MAX_NCUT_UNROLLED = 8;
+
+struct PairConsts {
+    double L;                 // period
+    double halfL;
+    double c2nL[MAX_NCUT_UNROLLED + 1];   // 2 n L
+    double n2L2[MAX_NCUT_UNROLLED + 1];   // (n L)^2
+};
+
+struct DevFlags {             // written by pack_kernel, read by the pair kernels
+    unsigned long long hmax_bits;   // bit pattern of max_i h_i (positive doubles order as integers)
+    int bad_h;                      // some h_i <= 0 or NaN
+    int pad;
+};
+
+__device__ __forceinline__ double rsqrt_seed(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));   // MUFU.RSQ64H: 20-bit, low word 0
+    return y;
+}
+
+// (x)^(-3/2) for normal positive x, ~1.5 ulp.  Series remainder 35/16 e^3 < 2^-56 for |e| < 2^-19.
+__device__ __forceinline__ double inv_cube_sqrt(double x)
+{
+    const double y0 = rsqrt_seed(x);
+    const double y2 = y0 * y0;                 // exact (21-bit operands)
+    const double e  = fma(-x, y2, 1.0);
+    const double c  = y2 * y0;
+    const double p  = fma(1.875, e, 1.5);
+    return fma(c * e, p, c);
+}
+
+// w = F(s, h)/s of Eq. 3 for s^2 = q < h^2, h = h_i + h_j  (slow path).
+__device__ __noinline__ double spline_w(double q, double hh)
+{
+    const double s   = sqrt(q);
+    const double ih  = 1.0 / hh;
+    const double u   = s * ih;
+    const double ih3 = ih * ih * ih;
+    if (u < 0.5)
+        return fma(u * u, fma(32.0, u, -38.4), 32.0 / 3.0) * ih3;
+    const double u3 = u * u * u;
+    double poly = fma(u, fma(u, fma(u, -32.0 / 3.0, 38.4), -48.0), 64.0 / 3.0);
+    poly -= 1.0 / (15.0 * u3);
+    return poly * ih3;
+}
+
+// One source j against one target i: adds into (ax, ay, az1, az2).
+// NC > 0: image loop fully unrolled for N_cut == NC; NC == 0: run-time N_cut.
+template <int NC>
+__device__ __forceinline__ void pair_term(double xi, double yi, double zi, double hi,
+                                          double xj, double yj, double zj, double mj, double hj,
+                                          const PairConsts &k, int ncut_rt,
+                                          double &ax, double &ay, double &az1, double &az2)
+{
+    const double rx = xi - xj, ry = yi - yj;
+    double rz = zi - zj;                                   // in (-L, L): both z in [0, L)
+    const double shift = (fabs(rz) > k.halfL) ? copysign(k.L, rz) : 0.0;
+    rz -= shift;                                           // nearest image, |rz| <= L/2
+    const double rho2 = fma(ry, ry, rx * rx);
+    const double q = fma(rz, rz, rho2);
+    const double hh = hi + hj;
+
+    // nearest image n = 0 (the only one the spline can touch on this path)
+    double w0 = inv_cube_sqrt(q);
+    if (q < hh * hh) w0 = spline_w(q, hh);
+    double S = w0, T = 0.0;
+
+    if (NC > 0) {
+#pragma unroll
+        for (int n = 1; n < NC; ++n) {
+            const double B  = q + k.n2L2[n];
+            const double wp = inv_cube_sqrt(fma(-k.c2nL[n], rz, B));   // image +n: d = rz - nL
+            const double wm = inv_cube_sqrt(fma(k.c2nL[n], rz, B));    // image -n: d = rz + nL
+            S += wp;
+            S += wm;
+            T = fma((double)n, wp - wm, T);
+        }
+        // end image n = sign(rz) N_cut (absent when rz == 0): d = -sign(rz)(N L - |rz|)
+        double we = inv_cube_sqrt(fma(-k.c2nL[NC], fabs(rz), q + k.n2L2[NC]));
+        we = (rz == 0.0) ? 0.0 : we;
+        S += we;
+        T = fma(copysign((double)NC, rz), we, T);
+    } else {
+        for (int n = 1; n < ncut_rt; ++n) {
+            const double nL = (double)n * k.L;
+            const double B  = fma(nL, nL, q);
+            const double t  = 2.0 * nL;
+            const double wp = inv_cube_sqrt(fma(-t, rz, B));
+            const double wm = inv_cube_sqrt(fma(t, rz, B));
+            S += wp;
+            S += wm;
+            T = fma((double)n, wp - wm, T);
+        }
+        const double NL = (double)ncut_rt * k.L;
+        double we = inv_cube_sqrt(fma(-2.0 * NL, fabs(rz), fma(NL, NL, q)));
+        we = (rz == 0.0) ? 0.0 : we;
+        S += we;
+        T = fma(copysign((double)ncut_rt, rz), we, T);
+    }
+    const double Sm = mj * S;
+    ax  = fma(Sm, rx, ax);
+    ay  = fma(Sm, ry, ay);
+    az1 = fma(Sm, rz, az1);
+    az2 = fma(mj, T, az2);
+}
+
+// General path (2 max(h) > L/2): every image is formed directly and sent through the
+// spline test, exactly as Eq. 8 is written.
+__device__ __forceinline__ void pair_term_general(double xi, double yi, double zi, double hi,
+                                                  double xj, double yj, double zj, double mj,
+                                                  double hj, const PairConsts &k, int ncut,
+                                                  double &ax, double &ay, double &az1, double &az2)
+{
+    const double rx = xi - xj, ry = yi - yj;
+    double rz = zi - zj;
+    const double shift = (fabs(rz) > k.halfL) ? copysign(k.L, rz) : 0.0;
+    rz -= shift;
+    const double rho2 = fma(ry, ry, rx * rx);
+    const double hh = hi + hj, hh2 = hh * hh;
+    int nlo = -ncut + 1, nhi = ncut - 1;
+    if (rz > 0.0) nhi = ncut;
+    if (rz < 0.0) nlo = -ncut;
+    double S = 0.0, T = 0.0;
+    for (int n = nlo; n <= nhi; ++n) {
+        const double d = rz - (double)n * k.L;
+        const double s2 = fma(d, d, rho2);
+        double w = (s2 < hh2) ? spline_w(s2, hh) : inv_cube_sqrt(s2);
+        S += w;
+        T = fma((double)n, w, T);
+    }
+    const double Sm = mj * S;
+    ax  = fma(Sm, rx, ax);
+    ay  = fma(Sm, ry, ay);
+    az1 = fma(Sm, rz, az1);
+    az2 = fma(mj, T, az2);
+}
+
+// Packed source layout (written by pack_kernel, padded to a multiple of PAIR_THREADS with
+// massless far-away dummies): xy[j] = {x, y}, zm[j] = {z in [0,L), m}, hs[j] = h.
+//
+// grid = (ceil(n / PAIR_THREADS), n_chunks); CTA (bx, by) handles targets
+// [bx*128, bx*128+128) against source tiles [by*tiles_per_chunk, (by+1)*tiles_per_chunk).
+// part layout: part[((chunk*4 + comp) * n_pad) + i].
+// MODE: 0 = fast path (exits at once if the general path is required), 1 = general path
+// (exits at once if it is not).
+template <int NC, int MODE>
+__global__ void __launch_bounds__(PAIR_THREADS)
+pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                 const double *__restrict__ hs, int n_pad, int n_tiles, int tiles_per_chunk,
+                 int ncut_rt, PairConsts k, const DevFlags *__restrict__ flags,
+                 double *__restrict__ part)
+{
+    {
+        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
+        const bool need_general = (2.0 * hmax > k.halfL) || flags->bad_h;
+        if (need_general != (MODE == 1)) return;
+    }
+    __shared__ double2 s_xy[PAIR_THREADS];
+    __shared__ double2 s_zm[PAIR_THREADS];
+    __shared__ double  s_h[PAIR_THREADS];
+
+    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;      // < n_pad always
+    const double2 pi = xy[i], qi = zm[i];
+    const double xi = pi.x, yi = pi.y, zi = qi.x, hi = hs[i];
+    double ax = 0.0, ay = 0.0, az1 = 0.0, az2 = 0.0;
+
+    const int t0 = blockIdx.y * tiles_per_chunk;
+    const int t1 = min(t0 + tiles_per_chunk, n_tiles);
+    for (int t = t0; t < t1; ++t) {
+        const int j = t * PAIR_THREADS + threadIdx.x;
+        __syncthreads();
+        s_xy[threadIdx.x] = xy[j];
+        s_zm[threadIdx.x] = zm[j];
+        s_h[threadIdx.x]  = hs[j];
+        __syncthreads();
+#pragma unroll 1
+        for (int jj = 0; jj < PAIR_THREADS; ++jj) {
+            const double2 a = s_xy[jj], b = s_zm[jj];
+            const double hj = s_h[jj];
+            if (MODE == 0)
+                pair_term<NC>(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt, ax, ay, az1, az2);
+            else
+                pair_term_general(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt,
+                                  ax, ay, az1, az2);
+        }
+    }
+    double *p = part + (size_t)blockIdx.y * 4 * n_pad + i;
+    p[0] = ax;
+    p[(size_t)n_pad] = ay;
+    p[2 * (size_t)n_pad] = az1;
+    p[3 * (size_t)n_pad] = az2;
+}
+
+}  // namespace steps

@@ -1,0 +1,448 @@
+// steps_cyl.cu -- host side of libsteps_cyl.so: context, validation, scratch ownership, kernel
+// launches, and the C ABI declared in include/steps_cyl.h.  No torch types, no CPU fallback.
+#include "../../include/steps_cyl.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "aux_kernels.cuh"
+#include "pair_fp64.cuh"
+#include "pair_mixed.cuh"
+
+using namespace steps;
+
+struct steps_cyl_ctx {
+    steps_cyl_params p;
+    int n, n_pad, n_tiles;
+    int n_chunks, tiles_per_chunk;
+    int sm_count;
+    PairConsts kc;
+    MixedConsts mc;
+    // device scratch (owned)
+    double2 *xy = nullptr, *zm = nullptr;
+    double *hs = nullptr;
+    float4 *f_hi = nullptr, *f_lo = nullptr;
+    double *part = nullptr;
+    double *bx = nullptr, *by = nullptr;          // background acceleration at the current x
+    DevFlags *flags = nullptr;
+    QuadNode *nodes = nullptr;
+    int n_nodes = 0;
+    double *host_io = nullptr;                     // device staging for the *_host entry points
+    double *peak_out = nullptr;
+    cudaStream_t own_stream = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    bool bg_valid = false;                         // bx/by hold b(x) for the caller's current x
+    int64_t launches = 0;
+    char cuda_msg[256];
+};
+
+namespace {
+
+int cuda_fail(steps_cyl_ctx *c, cudaError_t e)
+{
+    if (c) snprintf(c->cuda_msg, sizeof c->cuda_msg, "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return STEPS_ECUDA;
+}
+
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_);            \
+    } while (0)
+
+template <typename T>
+cudaError_t dev_alloc(T **p, size_t count)
+{
+    return cudaMalloc((void **)p, count * sizeof(T));
+}
+
+// Double-exponential (tanh-sinh) nodes on [0, R]: Y = R/2 (1 + tanh(pi/2 sinh t)), stored with
+// the distance to the nearer end point computed without cancellation.
+std::vector<QuadNode> make_nodes(double R)
+{
+    std::vector<QuadNode> v;
+    const double step = 1.0 / 16.0, half = 0.5 * R, hpi = 1.57079632679489661923;
+    for (int k = -120; k <= 120; ++k) {
+        const double t = k * step;
+        const double u = hpi * std::sinh(t);
+        const double ch = std::cosh(u);
+        const double wgt = step * half * hpi * std::cosh(t) / (ch * ch);
+        const double d = half * std::exp(-std::fabs(u)) / ch;       // distance to nearer end
+        if (!(wgt > 0.0) || !(d > 0.0) || wgt < 1e-40 * R) continue;
+        QuadNode q;
+        if (u >= 0.0) { q.Y = R - d; q.e = d; }                      // near Y = R
+        else          { q.Y = d;     q.e = R - d; }                  // near Y = 0
+        q.wgt = wgt;
+        v.push_back(q);
+    }
+    return v;
+}
+
+void choose_chunks(steps_cyl_ctx *c)
+{
+    // Enough CTAs for ~24 waves of 4 resident CTAs per SM, at least one source tile per chunk.
+    const int i_blocks = c->n_tiles;
+    const int target = 24 * 4 * c->sm_count;
+    int chunks = (target + i_blocks - 1) / i_blocks;
+    chunks = std::max(1, std::min(chunks, c->n_tiles));
+    chunks = std::min(chunks, 64);
+    c->tiles_per_chunk = (c->n_tiles + chunks - 1) / chunks;
+    c->n_chunks = (c->n_tiles + c->tiles_per_chunk - 1) / c->tiles_per_chunk;
+}
+
+template <int NC>
+void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    dim3 grid(c->n_tiles, c->n_chunks);
+    pair_fp64_kernel<NC, 0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->n_pad, c->n_tiles,
+                                                         c->tiles_per_chunk, c->p.n_cut, c->kc,
+                                                         c->flags, c->part);
+}
+
+template <int NC>
+void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    dim3 grid(c->n_tiles, c->n_chunks);
+    pair_mixed_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->n_pad, c->n_tiles,
+                                                       c->tiles_per_chunk, c->p.n_cut, c->mc,
+                                                       c->kc.halfL, c->flags, c->part);
+}
+
+void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
+{
+    const bool mixed = c->p.precision == STEPS_PREC_MIXED;
+    switch (c->p.n_cut) {
+#define CASE_NC(N)                                               \
+    case N:                                                      \
+        if (mixed) launch_pair_mixed_nc<N>(c, s);                \
+        else launch_pair_fp64_nc<N>(c, s);                       \
+        break;
+        CASE_NC(1) CASE_NC(2) CASE_NC(3) CASE_NC(4) CASE_NC(5) CASE_NC(6) CASE_NC(7) CASE_NC(8)
+#undef CASE_NC
+    default:
+        if (mixed) launch_pair_mixed_nc<0>(c, s);
+        else launch_pair_fp64_nc<0>(c, s);
+    }
+    // general path: a no-op unless 2 max(h) > L/2
+    dim3 grid(c->n_tiles, c->n_chunks);
+    pair_fp64_kernel<0, 1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->n_pad, c->n_tiles,
+                                                        c->tiles_per_chunk, c->p.n_cut, c->kc,
+                                                        c->flags, c->part);
+    c->launches += 2;
+}
+
+int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z,
+                  const double *m, const double *h, double *gx, double *gy, double *gz,
+                  cudaStream_t s)
+{
+    const int tb = 256;
+    CK(cudaMemsetAsync(ctx->flags, 0, sizeof(DevFlags), s));
+    pack_kernel<<<(ctx->n_pad + tb - 1) / tb, tb, 0, s>>>(x, y, z, m, h, ctx->n, ctx->n_pad,
+                                                         ctx->p.Lz, ctx->xy, ctx->zm, ctx->hs,
+                                                         ctx->f_hi, ctx->f_lo, ctx->flags);
+    ctx->launches += 1;
+    CK(cudaEventRecord(ctx->ev0, s));
+    launch_pair(ctx, s);
+    CK(cudaEventRecord(ctx->ev1, s));
+    ctx->ev_valid = true;
+    finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
+                                                         ctx->n_chunks, ctx->p.G, ctx->p.Lz, gx, gy, gz);
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int enqueue_background(steps_cyl_ctx *ctx, const double *x, const double *y, double *bx, double *by,
+                       cudaStream_t s)
+{
+    const int tb = 128;
+    background_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(
+        x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0,
+        ctx->p.background == STEPS_BG_INFINITE, ctx->nodes, ctx->n_nodes, bx, by);
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return STEPS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
+{
+    if (!p || !out) return STEPS_EINVAL;
+    *out = nullptr;
+    if (p->n < 1 || p->n >= (int64_t)2147483647 - 2 * PAIR_THREADS) return STEPS_EINVAL;
+    if (!(p->Lz > 0.0) || !std::isfinite(p->Lz) || !std::isfinite(p->G)) return STEPS_EINVAL;
+    if (p->n_cut < 1 || p->n_cut > 1000000) return STEPS_EINVAL;
+    if (p->periodic_mode == STEPS_PERIODIC_EWALD_TABLE) return STEPS_EUNSUPPORTED;
+    if (p->periodic_mode != STEPS_PERIODIC_IMAGES) return STEPS_EINVAL;
+    if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
+    if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
+    if (p->reserved != 0 || p->device < 0) return STEPS_EINVAL;
+    if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
+    if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
+
+    steps_cyl_ctx *ctx = new (std::nothrow) steps_cyl_ctx();
+    if (!ctx) return STEPS_ENOMEM;
+    ctx->cuda_msg[0] = 0;
+    ctx->p = *p;
+    int rc = STEPS_OK;
+    auto fail = [&](int code) { steps_cyl_destroy(ctx); return code; };
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device >= ndev) { delete ctx; return STEPS_ECUDA; }
+    if (cudaSetDevice(p->device) != cudaSuccess) { delete ctx; return STEPS_ECUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) { delete ctx; return STEPS_ECUDA; }
+    ctx->sm_count = prop.multiProcessorCount;
+
+    ctx->n = (int)p->n;
+    ctx->n_tiles = (ctx->n + PAIR_THREADS - 1) / PAIR_THREADS;
+    ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
+    choose_chunks(ctx);
+
+    const double L = p->Lz;
+    ctx->kc.L = L;
+    ctx->kc.halfL = 0.5 * L;
+    ctx->mc.Lh = (float)L;
+    ctx->mc.Ll = (float)(L - (double)ctx->mc.Lh);
+    ctx->mc.halfL = (float)(0.5 * L);
+    for (int n = 0; n <= MAX_NCUT_UNROLLED; ++n) {
+        const double nL = (double)n * L;
+        ctx->kc.c2nL[n] = 2.0 * nL;
+        ctx->kc.n2L2[n] = nL * nL;
+        ctx->mc.c2nL[n] = (float)(2.0 * nL);
+        ctx->mc.n2L2[n] = (float)(nL * nL);
+    }
+
+    auto A = [&](cudaError_t e) { if (e != cudaSuccess && rc == STEPS_OK) { rc = (e == cudaErrorMemoryAllocation) ? STEPS_ENOMEM : STEPS_ECUDA; cuda_fail(ctx, e); } };
+    const size_t np = (size_t)ctx->n_pad;
+    A(dev_alloc(&ctx->xy, np));
+    A(dev_alloc(&ctx->zm, np));
+    A(dev_alloc(&ctx->hs, np));
+    A(dev_alloc(&ctx->f_hi, np));
+    A(dev_alloc(&ctx->f_lo, np));
+    A(dev_alloc(&ctx->part, np * 4 * (size_t)ctx->n_chunks));
+    A(dev_alloc(&ctx->bx, np));
+    A(dev_alloc(&ctx->by, np));
+    A(dev_alloc(&ctx->flags, 1));
+    A(dev_alloc(&ctx->peak_out, 1));
+    A(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+    A(cudaEventCreate(&ctx->ev0));
+    A(cudaEventCreate(&ctx->ev1));
+    if (rc != STEPS_OK) return fail(rc);
+
+    if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE) {
+        std::vector<QuadNode> v = make_nodes(p->R_sim);
+        ctx->n_nodes = (int)v.size();
+        A(dev_alloc(&ctx->nodes, v.size()));
+        if (rc == STEPS_OK) A(cudaMemcpy(ctx->nodes, v.data(), v.size() * sizeof(QuadNode), cudaMemcpyHostToDevice));
+        if (rc != STEPS_OK) return fail(rc);
+    }
+    A(cudaMemset(ctx->flags, 0, sizeof(DevFlags)));
+    if (rc != STEPS_OK) return fail(rc);
+    *out = ctx;
+    return STEPS_OK;
+}
+
+void steps_cyl_destroy(steps_cyl_ctx *c)
+{
+    if (!c) return;
+    cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->f_hi); cudaFree(c->f_lo);
+    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes);
+    cudaFree(c->host_io); cudaFree(c->peak_out);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    delete c;
+}
+
+int steps_cyl_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z,
+                    const double *m, const double *h, double *gx, double *gy, double *gz,
+                    void *cuda_stream)
+{
+    if (!ctx || !x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    return enqueue_accel(ctx, x, y, z, m, h, gx, gy, gz, (cudaStream_t)cuda_stream);
+}
+
+int steps_cyl_check(steps_cyl_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    CK(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    DevFlags f;
+    CK(cudaMemcpy(&f, ctx->flags, sizeof f, cudaMemcpyDeviceToHost));
+    CK(cudaGetLastError());
+    return f.bad_h ? STEPS_ESOFT : STEPS_OK;
+}
+
+int steps_cyl_accel_host(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z,
+                         const double *m, const double *h, double *gx, double *gy, double *gz)
+{
+    if (!ctx || !x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    const size_t n = (size_t)ctx->n, B = n * sizeof(double);
+    if (!ctx->host_io) {
+        cudaError_t e = dev_alloc(&ctx->host_io, 11 * n);
+        if (e != cudaSuccess) { cuda_fail(ctx, e); return e == cudaErrorMemoryAllocation ? STEPS_ENOMEM : STEPS_ECUDA; }
+    }
+    cudaStream_t s = ctx->own_stream;
+    double *d = ctx->host_io;
+    const double *src[5] = {x, y, z, m, h};
+    for (int k = 0; k < 5; ++k) CK(cudaMemcpyAsync(d + k * n, src[k], B, cudaMemcpyHostToDevice, s));
+    int rc = enqueue_accel(ctx, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d + 7 * n, s);
+    if (rc != STEPS_OK) return rc;
+    double *dst[3] = {gx, gy, gz};
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], d + (5 + k) * n, B, cudaMemcpyDeviceToHost, s));
+    return steps_cyl_check(ctx, (void *)s);
+}
+
+int steps_cyl_background(steps_cyl_ctx *ctx, const double *x, const double *y, double *bx, double *by,
+                         void *cuda_stream)
+{
+    if (!ctx || !x || !y || !bx || !by) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    return enqueue_background(ctx, x, y, bx, by, (cudaStream_t)cuda_stream);
+}
+
+int steps_cyl_kdk_step(steps_cyl_ctx *ctx, double *x, double *y, double *z, double *vx, double *vy,
+                       double *vz, const double *m, const double *h, double *gx, double *gy,
+                       double *gz, double a_n, double H_n, double a_np1, double H_np1, double dt,
+                       void *cuda_stream)
+{
+    if (!ctx || !x || !y || !z || !vx || !vy || !vz || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
+    if (!(a_n > 0.0) || !(a_np1 > 0.0) || !std::isfinite(dt)) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int tb = 256, nb = (ctx->n + tb - 1) / tb;
+    // b(x_n): the caller may have moved the particles since the last step, so it is recomputed
+    // (O(N), ~1e-3 of the pair sum).
+    int rc = enqueue_background(ctx, x, y, ctx->bx, ctx->by, s);
+    if (rc != STEPS_OK) return rc;
+    kick1_drift_kernel<<<nb, tb, 0, s>>>(x, y, z, vx, vy, vz, gx, gy, gz, ctx->bx, ctx->by, ctx->n,
+                                         1.0 / (a_n * a_n * a_n), H_n, dt, ctx->p.Lz);
+    ctx->launches += 1;
+    rc = enqueue_accel(ctx, x, y, z, m, h, gx, gy, gz, s);
+    if (rc != STEPS_OK) return rc;
+    rc = enqueue_background(ctx, x, y, ctx->bx, ctx->by, s);
+    if (rc != STEPS_OK) return rc;
+    kick2_kernel<<<nb, tb, 0, s>>>(vx, vy, vz, gx, gy, gz, ctx->bx, ctx->by, ctx->n,
+                                   1.0 / (a_np1 * a_np1 * a_np1), H_np1, dt);
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx, double *x, double *y, double *z, double *vx,
+                            double *vy, double *vz, const double *m, const double *h, double *gx,
+                            double *gy, double *gz, double a_n, double H_n, double a_np1,
+                            double H_np1, double dt)
+{
+    if (!ctx || !x || !y || !z || !vx || !vy || !vz || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    const size_t n = (size_t)ctx->n, B = n * sizeof(double);
+    if (!ctx->host_io) {
+        cudaError_t e = dev_alloc(&ctx->host_io, 11 * n);
+        if (e != cudaSuccess) { cuda_fail(ctx, e); return e == cudaErrorMemoryAllocation ? STEPS_ENOMEM : STEPS_ECUDA; }
+    }
+    cudaStream_t s = ctx->own_stream;
+    double *d = ctx->host_io;
+    const double *src[11] = {x, y, z, vx, vy, vz, m, h, gx, gy, gz};
+    for (int k = 0; k < 11; ++k) CK(cudaMemcpyAsync(d + k * n, src[k], B, cudaMemcpyHostToDevice, s));
+    int rc = steps_cyl_kdk_step(ctx, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n,
+                                d + 7 * n, d + 8 * n, d + 9 * n, d + 10 * n, a_n, H_n, a_np1, H_np1,
+                                dt, (void *)s);
+    if (rc != STEPS_OK) return rc;
+    double *dst[11] = {x, y, z, vx, vy, vz, nullptr, nullptr, gx, gy, gz};
+    for (int k = 0; k < 11; ++k)
+        if (dst[k]) CK(cudaMemcpyAsync(dst[k], d + k * n, B, cudaMemcpyDeviceToHost, s));
+    return steps_cyl_check(ctx, (void *)s);
+}
+
+static double hubble_of_a(double a, double H0, double Om, double Or, double Ok, double OL)
+{
+    const double ia = 1.0 / a;
+    return H0 * std::sqrt(((Or * ia + Om) * ia + Ok) * ia * ia + OL);
+}
+
+int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double Or, double Ok,
+                             double OL, double *a_next, double *H_next)
+{
+    if (!a_next || !H_next || !(a > 0.0)) return STEPS_EINVAL;
+    auto f = [&](double s) { return s * hubble_of_a(s, H0, Om, Or, Ok, OL); };
+    const double k1 = f(a);
+    const double k2 = f(a + 0.5 * dt * k1);
+    const double k3 = f(a + 0.5 * dt * k2);
+    const double k4 = f(a + dt * k3);
+    const double an = a + dt / 6.0 * (k1 + 2.0 * (k2 + k3) + k4);
+    *a_next = an;
+    *H_next = hubble_of_a(an, H0, Om, Or, Ok, OL);
+    return STEPS_OK;
+}
+
+int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s)
+{
+    if (!ctx || !dfma_per_s || !(ms > 0.0)) return STEPS_EINVAL;
+    CK(cudaSetDevice(ctx->p.device));
+    cudaStream_t s = ctx->own_stream;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const int blocks = ctx->sm_count * 8, threads = 256;
+    int iters = 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CK(cudaEventRecord(e0, s));
+        dfma_peak_kernel<<<blocks, threads, 0, s>>>(ctx->peak_out, iters, 0.999999, 1.0e-3);
+        CK(cudaEventRecord(e1, s));
+        CK(cudaEventSynchronize(e1));
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, e0, e1));
+        ctx->launches += 1;
+        const double rate = (double)blocks * threads * 16.0 * iters / (t * 1e-3);
+        if (rep > 0) best = std::max(best, rate);
+        // aim the next repetition at `ms`
+        const double scale = ms / std::max((double)t, 1e-3);
+        iters = (int)std::min(4.0e6, std::max(1024.0, iters * scale));
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *dfma_per_s = best;
+    return STEPS_OK;
+}
+
+int steps_cyl_last_pair_kernel_ms(steps_cyl_ctx *ctx, float *ms)
+{
+    if (!ctx || !ms || !ctx->ev_valid) return STEPS_EINVAL;
+    CK(cudaEventSynchronize(ctx->ev1));
+    CK(cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1));
+    return STEPS_OK;
+}
+
+const char *steps_cyl_strerror(int code)
+{
+    switch (code) {
+    case STEPS_OK: return "ok";
+    case STEPS_EINVAL: return "invalid argument";
+    case STEPS_ESOFT: return "softening precondition violated (some h_i <= 0)";
+    case STEPS_ECUDA: return "CUDA runtime error (see steps_cyl_last_cuda_error)";
+    case STEPS_ENOMEM: return "out of memory";
+    case STEPS_EUNSUPPORTED: return "mode not built (EWALD_TABLE)";
+    default: return "unknown status";
+    }
+}
+
+const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx) { return ctx ? ctx->cuda_msg : ""; }
+
+int64_t steps_cyl_launch_count(steps_cyl_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,129 @@
+"""GPU-vs-oracle parity of the O(N) parts of the path through the C ABI: the homogeneous-cylinder
+background term (Eq. 9/10, steps_cyl_background) and the KDK leapfrog step of Eq. 11
+(steps_cyl_kdk_step), plus the config-3 trajectory at reduced N."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200; there is no CPU fallback"
+    return torch
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_background_matches_oracle(torch_cuda, oracle, mode):
+    from paper_2602_20787_b200 import binding as b
+    torch = torch_cuda
+    rng = np.random.default_rng(5)
+    n, R, L, ncut, G, rho0 = 4000, 1000.0, 100.0, 5, 4.30091e-9, 8.3e10
+    r = np.concatenate([R * np.sqrt(rng.random(n - 8)),
+                        [0.0, 1e-9, R, R * (1 - 1e-12), R * (1 + 1e-9), 0.999 * R, 1.001 * R, 1.2 * R]])
+    phi = 2 * np.pi * rng.random(n)
+    x, y = r * np.cos(phi), r * np.sin(phi)
+    ctx = b.StepsCyl(n=n, Lz=L, G=G, n_cut=ncut, background=mode, R_sim=R, rho0=rho0)
+    bx = torch.empty(n, dtype=torch.float64, device="cuda")
+    by = torch.empty_like(bx)
+    ctx.background(_dev(torch, x), _dev(torch, y), bx, by)
+    ctx.check()
+    rx, ry = oracle.background(x, y, R, ncut * L, G, rho0, mode)
+    scale = np.abs(np.hypot(rx, ry)).max()
+    assert np.abs(bx.cpu().numpy() - rx).max() <= 2e-11 * scale
+    assert np.abs(by.cpu().numpy() - ry).max() <= 2e-11 * scale
+    # outward push (Eq. 11 subtracts F_h < 0)
+    assert np.all((bx.cpu().numpy() * x + by.cpu().numpy() * y)[r > 1e-6] > 0)
+    ctx.close()
+
+
+def _kdk_both(torch, oracle, w, n_steps, background):
+    """Run n_steps of KDK on the GPU and in the oracle from the same start; returns both states."""
+    from paper_2602_20787_b200 import binding as b
+    c = w.cosmo
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=w.n_cut, background=background, R_sim=w.R_sim,
+                     rho0=w.rho0)
+    names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
+    host = {k: np.ascontiguousarray(getattr(w, k), dtype=np.float64).copy() for k in names}
+    dev = {k: _dev(torch, host[k]) for k in names}
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+    og = list(oracle.accel(host["x"], host["y"], host["z"], host["m"], host["h"], w.Lz, w.G, w.n_cut))
+    a = c["a_init"]
+    H = oracle.hubble(a, c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+    for _ in range(n_steps):
+        a1, H1 = b.friedmann_step(a, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+        oa1, oH1 = oracle.friedmann_rk4(a, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+        assert a1 == pytest.approx(oa1, rel=1e-14) and H1 == pytest.approx(oH1, rel=1e-14)
+        ctx.kdk_step(*[dev[k] for k in names], *g, a, H, a1, H1, c["dt"])
+        oracle.kdk_step(*[host[k] for k in names], *og, w.Lz, w.G, w.n_cut, w.R_sim, w.rho0,
+                        background, a, H, oa1, oH1, c["dt"])
+        a, H = a1, H1
+    ctx.check()
+    out = {k: dev[k].cpu().numpy() for k in names}
+    gg = [t.cpu().numpy() for t in g]
+    ctx.close()
+    return out, gg, host, og, a
+
+
+@pytest.mark.parametrize("background", [0, 1])
+def test_one_kdk_step_matches_oracle(torch_cuda, oracle, background):
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(3, n=3000)
+    out, g, ref, og, _ = _kdk_both(torch_cuda, oracle, w, 1, background)
+    for k in ("x", "y"):
+        assert np.abs(out[k] - ref[k]).max() <= 1e-12 * np.abs(ref[k]).max()
+    dz = out["z"] - ref["z"]
+    dz -= w.Lz * np.rint(dz / w.Lz)
+    assert np.abs(dz).max() <= 1e-12 * w.Lz
+    for k in ("vx", "vy", "vz"):
+        assert np.abs(out[k] - ref[k]).max() <= 1e-10 * np.abs(ref[k]).max()
+    e = np.linalg.norm(np.stack(g, 1) - np.stack(og, 1), axis=1) / np.linalg.norm(np.stack(og, 1), axis=1)
+    assert e.max() <= 1e-10
+
+
+def test_config3_trajectory_reduced_n(torch_cuda, oracle):
+    """Config 3 (LCDM, a: 0.02 -> 0.025, 10 KDK steps) at N = 16384: the oracle integrates
+    independently; positions, velocities and final accelerations agree."""
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(3, n=16384)
+    out, g, ref, og, a_end = _kdk_both(torch_cuda, oracle, w, w.cosmo["n_steps"], 0)
+    assert a_end == pytest.approx(w.cosmo["a_final"], rel=1e-6)
+    for k in ("x", "y"):
+        assert np.abs(out[k] - ref[k]).max() <= 1e-10 * np.abs(ref[k]).max()
+    for k in ("vx", "vy", "vz"):
+        assert np.abs(out[k] - ref[k]).max() <= 1e-8 * np.abs(ref[k]).max()
+    e = np.linalg.norm(np.stack(g, 1) - np.stack(og, 1), axis=1) / np.linalg.norm(np.stack(og, 1), axis=1)
+    assert e.max() <= 1e-8        # accumulated round-off of 10 steps feeds back through positions
+
+
+def test_free_streaming_conserves_a2v(torch_cuda):
+    """g = 0 (G = 0), no background: a^2 v is conserved to O(dt^2) (reading S4 pin)."""
+    from paper_2602_20787_b200 import binding as b
+    torch = torch_cuda
+    n, H0 = 256, 70.0
+    rng = np.random.default_rng(3)
+    errs = []
+    for nsteps in (20, 40):
+        ctx = b.StepsCyl(n=n, Lz=100.0, G=0.0, n_cut=2)
+        st = {k: _dev(torch, rng.random(n) * 50 + 1) for k in ("x", "y", "z", "m", "h")}
+        v0 = rng.normal(0, 1, n)
+        v = [_dev(torch, v0), _dev(torch, v0 * 0.5), _dev(torch, -v0)]
+        g = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        a0, a1 = 0.5, 0.6
+        t0, t1 = (2 / (3 * H0)) * a0 ** 1.5, (2 / (3 * H0)) * a1 ** 1.5
+        dt = (t1 - t0) / nsteps
+        a, H = a0, H0 * a0 ** -1.5
+        for _ in range(nsteps):
+            an, Hn = b.friedmann_step(a, dt, H0, 1.0)
+            ctx.kdk_step(st["x"], st["y"], st["z"], *v, st["m"], st["h"], *g, a, H, an, Hn, dt)
+            a, H = an, Hn
+        ctx.check()
+        errs.append(float(np.abs(v[0].cpu().numpy() * a * a / (v0 * a0 * a0) - 1).max()))
+        ctx.close()
+    assert errs[0] < 1e-3 and errs[1] < errs[0] / 3.5
