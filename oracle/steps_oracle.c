@@ -147,20 +147,22 @@ int oracle_max_threads(void)
 static double fh_integrand(double Y, double e, double rho, double R, double L)
 {
     double X = sqrt(fmax(e * (R + Y), 0.0));
-    double ap = R * R + rho * rho + 2.0 * rho * X;
-    double am = R * R + rho * rho - 2.0 * rho * X;
+    /* a+- = R^2 + rho^2 +- 2 rho X with R^2 = X^2 + Y^2, written as (rho +- X)^2 + Y^2: the same
+     * number, but free of the cancellation that a- suffers for rho ~ R near Y = 0 */
+    double ap = (rho + X) * (rho + X) + Y * Y;
+    double am = (rho - X) * (rho - X) + Y * Y;
     double wp = sqrt(L * L + ap), wm = sqrt(L * L + am);
     if (am <= 0.0) return 0.0;               /* single point rho = R, Y = 0: integrable */
-    return 2.0 * log((wp + L) / (wm + L)) - log(ap / am);
+    return 2.0 * log((wp + L) / (wm + L)) - (log(ap) - log(am));   /* ap/am may overflow at rho = R */
 }
 
 static double fh_integrand_inf(double Y, double e, double rho, double R)
 {
     double X = sqrt(fmax(e * (R + Y), 0.0));
-    double ap = R * R + rho * rho + 2.0 * rho * X;
-    double am = R * R + rho * rho - 2.0 * rho * X;
+    double ap = (rho + X) * (rho + X) + Y * Y;
+    double am = (rho - X) * (rho - X) + Y * Y;
     if (am <= 0.0) return 0.0;
-    return -log(ap / am);
+    return -(log(ap) - log(am));
 }
 
 /* tanh-sinh on [0,R]; doubles the node count until two levels agree to 1e-14. */

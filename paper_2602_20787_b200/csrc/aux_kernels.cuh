@@ -95,12 +95,14 @@ __global__ void background_kernel(const double *__restrict__ x, const double *__
     if (infinite) {
         Fh = -2.0 * 3.141592653589793238 * G * rho0 * rho;          // Eq. 10
     } else {
-        const double base = fma(R, R, rho * rho), L2 = Lhalf * Lhalf;
+        const double L2 = Lhalf * Lhalf;
         double acc = 0.0;
         for (int kq = 0; kq < n_nodes; ++kq) {
             const QuadNode q = nodes[kq];
             const double X  = sqrt(q.e * (R + q.Y));
-            const double ap = fma(2.0 * rho, X, base), am = fma(-2.0 * rho, X, base);
+            // a+- = (rho +- X)^2 + Y^2  (R^2 = X^2 + Y^2): no cancellation for rho ~ R, Y ~ 0
+            const double Y2 = q.Y * q.Y, sp = rho + X, sm = rho - X;
+            const double ap = fma(sp, sp, Y2), am = fma(sm, sm, Y2);
             if (am <= 0.0) continue;                                  // rho == R, Y == 0: measure zero
             const double wp = sqrt(L2 + ap), wm = sqrt(L2 + am);
             const double ratio = (wp + Lhalf) / (wm + Lhalf);

@@ -68,8 +68,8 @@ cudaError_t dev_alloc(T **p, size_t count)
 std::vector<QuadNode> make_nodes(double R)
 {
     std::vector<QuadNode> v;
-    const double step = 1.0 / 16.0, half = 0.5 * R, hpi = 1.57079632679489661923;
-    for (int k = -120; k <= 120; ++k) {
+    const double step = 1.0 / 24.0, half = 0.5 * R, hpi = 1.57079632679489661923;
+    for (int k = -180; k <= 180; ++k) {
         const double t = k * step;
         const double u = hpi * std::sinh(t);
         const double ch = std::cosh(u);

@@ -28,6 +28,27 @@ def test_Fh_matches_independent_quadrature(oracle, rho, R, Lh):
     assert got == pytest.approx(want, rel=2e-11)
 
 
+@pytest.mark.parametrize("rho", [999.99, 1000.0 * (1 - 1e-12), 1000.0, 1000.0 * (1 + 1e-9), 1001.0])
+def test_Fh_at_the_cylinder_edge_against_mpmath(oracle, rho):
+    """rho ~ R: a- = (rho - X)^2 + Y^2 nearly vanishes at Y = 0 (logarithmic end-point
+    singularity of Eq. 9's second integral).  30-digit tanh-sinh of the same integrand, with
+    break points crowding Y = 0, fixes the value; a cancellation-prone a- fails this at 1e-7."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    R, L = mp.mpf(1000), mp.mpf(500)
+    r = mp.mpf(rho)
+
+    def f(Y):
+        X = mp.sqrt(R * R - Y * Y)
+        ap, am = R * R + r * r + 2 * r * X, (r - X) ** 2 + Y * Y      # same a- as Eq. 9, R^2 = X^2 + Y^2
+        if am <= 0:
+            return mp.mpf(0)
+        return 2 * mp.log((mp.sqrt(L * L + ap) + L) / (mp.sqrt(L * L + am) + L)) - mp.log(ap / am)
+
+    want = 2 * mp.quad(f, [0, R * 1e-9, R * 1e-6, R * 1e-3, R / 4, R / 2, R * 0.9, R * 0.99, R * 0.999, R])
+    assert oracle.Fh(rho, 1000.0, 500.0, 1.0, 1.0) == pytest.approx(float(want), rel=1e-12)
+
+
 def test_Fh_brute_force_3d_monte_carlo(oracle):
     """Crude but assumption-free: Monte-Carlo sum of Newtonian pulls of uniformly sampled mass
     elements of the finite cylinder; fixes sign and overall factor of Eq. 9."""
