@@ -34,7 +34,9 @@ __device__ __forceinline__ float rsqrt_f32(float x)
 __device__ __forceinline__ float inv_cube_sqrt_f32(float x)
 {
     const float y = rsqrt_f32(x);
-    return y * y * y;
+    // explicit roundings: a product left open to FMA contraction would make w(+n) - w(-n) != 0
+    // for r_z = 0 (one side fused into the subtraction, the other rounded)
+    return __fmul_rn(__fmul_rn(y, y), y);
 }
 
 __device__ __noinline__ float spline_w_f32(float q, float hh)
