@@ -26,10 +26,10 @@ __global__ void pack_kernel(const double *__restrict__ x, const double *__restri
                             double2 *__restrict__ xy, double2 *__restrict__ zm,
                             double *__restrict__ hs,
                             float4 *__restrict__ f_hi, float4 *__restrict__ f_lo,
-                            DevFlags *__restrict__ flags)
+                            double *__restrict__ tile_hmax, DevFlags *__restrict__ flags)
 {
+    // launched with PAIR_THREADS threads per block: block b == source tile b (n_pad = tiles * 128)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_pad) return;
     double xv, yv, zv, mv, hv;
     if (i < n) {
         xv = x[i]; yv = y[i]; zv = wrap_z(z[i], L); mv = m[i]; hv = h[i];
@@ -41,6 +41,19 @@ __global__ void pack_kernel(const double *__restrict__ x, const double *__restri
     xy[i] = make_double2(xv, yv);
     zm[i] = make_double2(zv, mv);
     hs[i] = hv;
+    {   // max h of the tile (dummies count as 0): bounds h_i + h_j in the pair kernels' spline pre-test
+        __shared__ double s_max[PAIR_THREADS / 32];
+        double hm = (i < n && hv > 0.0) ? hv : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) hm = fmax(hm, __shfl_xor_sync(0xffffffffu, hm, o));
+        if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = hm;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = s_max[0];
+            for (int wq = 1; wq < PAIR_THREADS / 32; ++wq) t = fmax(t, s_max[wq]);
+            tile_hmax[blockIdx.x] = t;
+        }
+    }
     if (f_hi) {
         // x = hi + lo with hi = fl32(x), lo = fl32(x - hi): the difference of two such pairs,
         // (hi_i - hi_j) + (lo_i - lo_j), keeps ~2^-24 RELATIVE accuracy of the separation

@@ -33,6 +33,7 @@ constexpr int MAX_NCUT_UNROLLED = 8;
 struct PairConsts {
     double L;                 // period
     double halfL;
+    int L_hi, L_lo, halfL_hi; // integer views of L and L/2 (ALU-pipe wrap test)
     double c2nL[MAX_NCUT_UNROLLED + 1];   // 2 n L
     double n2L2[MAX_NCUT_UNROLLED + 1];   // (n L)^2
 };
@@ -76,27 +77,41 @@ __device__ __noinline__ double spline_w(double q, double hh)
     return poly * ih3;
 }
 
-// One source j against one target i: adds into (ax, ay, az1, az2).
+// Integer views of a double: the FP64 pipe is the bottleneck, so sign / magnitude tests that do
+// not need a rounded result are done on the ALU pipe (high-word compares of positive doubles
+// order like the doubles themselves).
+__device__ __forceinline__ int hi32(double v) { return __double2hiint(v); }
+__device__ __forceinline__ int lo32(double v) { return __double2loint(v); }
+
+// Pair geometry (a2): r = x_i - x_j with r_z brought to the nearest image.  The decision uses
+// the high word only: |r_z| may stay above L/2 by a relative 2^-20, which leaves the image SET
+// {d = r_z - nL : |d| < N_cut L} and every formula below unchanged (reading S2).
+__device__ __forceinline__ double nearest_image(double rz, const PairConsts &k)
+{
+    const int h = hi32(rz);
+    const bool wrap = (h & 0x7fffffff) > k.halfL_hi;
+    const int sh = wrap ? (k.L_hi | (h & 0x80000000)) : 0;     // copysign(L, rz) or 0
+    const int sl = wrap ? k.L_lo : 0;
+    return rz - __hiloint2double(sh, sl);
+}
+
+// Image sum of one pair (a3/a4): S = sum_n w_n, T = sum_n n w_n over the window of Eq. 8.
+// soft_hi: high word of an upper bound of (h_i + h_j)^2 over the source tile; only pairs with
+// hi32(q) <= soft_hi can be inside the spline support and take the exact test.
 // NC > 0: image loop fully unrolled for N_cut == NC; NC == 0: run-time N_cut.
 template <int NC>
-__device__ __forceinline__ void pair_term(double xi, double yi, double zi, double hi,
-                                          double xj, double yj, double zj, double mj, double hj,
-                                          const PairConsts &k, int ncut_rt,
-                                          double &ax, double &ay, double &az1, double &az2)
+__device__ __forceinline__ void image_sum(double rz, double q, double hi, double hj, int soft_hi,
+                                          const PairConsts &k, int ncut_rt, double &S, double &T)
 {
-    const double rx = xi - xj, ry = yi - yj;
-    double rz = zi - zj;                                   // in (-L, L): both z in [0, L)
-    const double shift = (fabs(rz) > k.halfL) ? copysign(k.L, rz) : 0.0;
-    rz -= shift;                                           // nearest image, |rz| <= L/2
-    const double rho2 = fma(ry, ry, rx * rx);
-    const double q = fma(rz, rz, rho2);
-    const double hh = hi + hj;
-
     // nearest image n = 0 (the only one the spline can touch on this path)
     double w0 = inv_cube_sqrt(q);
-    if (q < hh * hh) w0 = spline_w(q, hh);
-    double S = w0, T = 0.0;
-
+    if (hi32(q) <= soft_hi) {
+        const double hh = hi + hj;
+        if (q < hh * hh) w0 = spline_w(q, hh);
+    }
+    S = w0;
+    T = 0.0;
+    const bool rz_nonzero = ((hi32(rz) & 0x7fffffff) | lo32(rz)) != 0;
     if (NC > 0) {
 #pragma unroll
         for (int n = 1; n < NC; ++n) {
@@ -105,13 +120,13 @@ __device__ __forceinline__ void pair_term(double xi, double yi, double zi, doubl
             const double wm = inv_cube_sqrt(fma(k.c2nL[n], rz, B));    // image -n: d = rz + nL
             S += wp;
             S += wm;
-            T = fma((double)n, wp - wm, T);
+            T = (n == 1) ? (wp - wm) : fma((double)n, wp - wm, T);
         }
         // end image n = sign(rz) N_cut (absent when rz == 0): d = -sign(rz)(N L - |rz|)
         double we = inv_cube_sqrt(fma(-k.c2nL[NC], fabs(rz), q + k.n2L2[NC]));
-        we = (rz == 0.0) ? 0.0 : we;
+        we = rz_nonzero ? we : 0.0;
         S += we;
-        T = fma(copysign((double)NC, rz), we, T);
+        T = (NC == 1) ? copysign(we, rz) : fma(copysign((double)NC, rz), we, T);
     } else {
         for (int n = 1; n < ncut_rt; ++n) {
             const double nL = (double)n * k.L;
@@ -125,10 +140,25 @@ __device__ __forceinline__ void pair_term(double xi, double yi, double zi, doubl
         }
         const double NL = (double)ncut_rt * k.L;
         double we = inv_cube_sqrt(fma(-2.0 * NL, fabs(rz), fma(NL, NL, q)));
-        we = (rz == 0.0) ? 0.0 : we;
+        we = rz_nonzero ? we : 0.0;
         S += we;
         T = fma(copysign((double)ncut_rt, rz), we, T);
     }
+}
+
+// One source j against one target i: adds into (ax, ay, az1, az2).
+template <int NC>
+__device__ __forceinline__ void pair_term(double xi, double yi, double zi, double hi,
+                                          double xj, double yj, double zj, double mj, double hj,
+                                          int soft_hi, const PairConsts &k, int ncut_rt,
+                                          double &ax, double &ay, double &az1, double &az2)
+{
+    const double rx = xi - xj, ry = yi - yj;
+    const double rz = nearest_image(zi - zj, k);          // zi - zj in (-L, L): both z in [0, L)
+    const double rho2 = fma(ry, ry, rx * rx);
+    const double q = fma(rz, rz, rho2);
+    double S, T;
+    image_sum<NC>(rz, q, hi, hj, soft_hi, k, ncut_rt, S, T);
     const double Sm = mj * S;
     ax  = fma(Sm, rx, ax);
     ay  = fma(Sm, ry, ay);
@@ -144,9 +174,7 @@ __device__ __forceinline__ void pair_term_general(double xi, double yi, double z
                                                   double &ax, double &ay, double &az1, double &az2)
 {
     const double rx = xi - xj, ry = yi - yj;
-    double rz = zi - zj;
-    const double shift = (fabs(rz) > k.halfL) ? copysign(k.L, rz) : 0.0;
-    rz -= shift;
+    const double rz = nearest_image(zi - zj, k);
     const double rho2 = fma(ry, ry, rx * rx);
     const double hh = hi + hj, hh2 = hh * hh;
     int nlo = -ncut + 1, nhi = ncut - 1;
@@ -178,9 +206,9 @@ __device__ __forceinline__ void pair_term_general(double xi, double yi, double z
 template <int NC, int MODE>
 __global__ void __launch_bounds__(PAIR_THREADS)
 pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
-                 const double *__restrict__ hs, int n_pad, int n_tiles, int tiles_per_chunk,
-                 int ncut_rt, PairConsts k, const DevFlags *__restrict__ flags,
-                 double *__restrict__ part)
+                 const double *__restrict__ hs, const double *__restrict__ tile_hmax, int n_pad,
+                 int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
+                 const DevFlags *__restrict__ flags, double *__restrict__ part)
 {
     {
         const double hmax = __longlong_as_double((long long)flags->hmax_bits);
@@ -205,12 +233,18 @@ pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
         s_zm[threadIdx.x] = zm[j];
         s_h[threadIdx.x]  = hs[j];
         __syncthreads();
+        int soft_hi;
+        {
+            const double b = hi + tile_hmax[t];          // >= h_i + h_j for every j of the tile
+            soft_hi = hi32(b * b);
+        }
 #pragma unroll 1
         for (int jj = 0; jj < PAIR_THREADS; ++jj) {
             const double2 a = s_xy[jj], b = s_zm[jj];
             const double hj = s_h[jj];
             if (MODE == 0)
-                pair_term<NC>(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt, ax, ay, az1, az2);
+                pair_term<NC>(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, soft_hi, k, ncut_rt, ax, ay, az1,
+                              az2);
             else
                 pair_term_general(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt,
                                   ax, ay, az1, az2);

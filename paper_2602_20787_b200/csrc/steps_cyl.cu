@@ -26,7 +26,7 @@ struct steps_cyl_ctx {
     MixedConsts mc;
     // device scratch (owned)
     double2 *xy = nullptr, *zm = nullptr;
-    double *hs = nullptr;
+    double *hs = nullptr, *tile_hmax = nullptr;
     float4 *f_hi = nullptr, *f_lo = nullptr;
     double *part = nullptr;
     double *bx = nullptr, *by = nullptr;          // background acceleration at the current x
@@ -101,7 +101,7 @@ template <int NC>
 void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles, c->n_chunks);
-    pair_fp64_kernel<NC, 0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->n_pad, c->n_tiles,
+    pair_fp64_kernel<NC, 0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
                                                          c->tiles_per_chunk, c->p.n_cut, c->kc,
                                                          c->flags, c->part);
 }
@@ -132,7 +132,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
     }
     // general path: a no-op unless 2 max(h) > L/2
     dim3 grid(c->n_tiles, c->n_chunks);
-    pair_fp64_kernel<0, 1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->n_pad, c->n_tiles,
+    pair_fp64_kernel<0, 1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
                                                         c->tiles_per_chunk, c->p.n_cut, c->kc,
                                                         c->flags, c->part);
     c->launches += 2;
@@ -144,9 +144,9 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
 {
     const int tb = 256;
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(DevFlags), s));
-    pack_kernel<<<(ctx->n_pad + tb - 1) / tb, tb, 0, s>>>(x, y, z, m, h, ctx->n, ctx->n_pad,
-                                                         ctx->p.Lz, ctx->xy, ctx->zm, ctx->hs,
-                                                         ctx->f_hi, ctx->f_lo, ctx->flags);
+    pack_kernel<<<ctx->n_tiles, PAIR_THREADS, 0, s>>>(x, y, z, m, h, ctx->n, ctx->n_pad, ctx->p.Lz,
+                                                     ctx->xy, ctx->zm, ctx->hs, ctx->f_hi, ctx->f_lo,
+                                                     ctx->tile_hmax, ctx->flags);
     ctx->launches += 1;
     CK(cudaEventRecord(ctx->ev0, s));
     launch_pair(ctx, s);
@@ -212,6 +212,15 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     const double L = p->Lz;
     ctx->kc.L = L;
     ctx->kc.halfL = 0.5 * L;
+    {
+        uint64_t bits;
+        std::memcpy(&bits, &L, 8);
+        ctx->kc.L_hi = (int)(bits >> 32);
+        ctx->kc.L_lo = (int)(bits & 0xffffffffu);
+        const double hl = 0.5 * L;
+        std::memcpy(&bits, &hl, 8);
+        ctx->kc.halfL_hi = (int)(bits >> 32);
+    }
     ctx->mc.Lh = (float)L;
     ctx->mc.Ll = (float)(L - (double)ctx->mc.Lh);
     ctx->mc.halfL = (float)(0.5 * L);
@@ -228,6 +237,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->xy, np));
     A(dev_alloc(&ctx->zm, np));
     A(dev_alloc(&ctx->hs, np));
+    A(dev_alloc(&ctx->tile_hmax, (size_t)ctx->n_tiles));
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
     A(dev_alloc(&ctx->part, np * 4 * (size_t)ctx->n_chunks));
@@ -256,7 +266,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
 void steps_cyl_destroy(steps_cyl_ctx *c)
 {
     if (!c) return;
-    cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->f_hi); cudaFree(c->f_lo);
+    cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
     cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
