@@ -66,6 +66,12 @@ enum { STEPS_PREC_FP64 = 0,            /* every pair term and the accumulation i
 enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz                                    */
        STEPS_BG_INFINITE = 1           /* Eq. 10                                                       */ };
 
+enum { STEPS_FLAG_DETERMINISTIC = 1    /* fp64 mode: evaluate every ORDERED pair and reduce in a fixed
+                                          order (bit-reproducible, ~1.9x slower) instead of the default
+                                          kernel, which evaluates every unordered pair once and applies
+                                          it to both particles with floating-point atomics (same terms,
+                                          summation order varies from run to run)                      */ };
+
 typedef struct steps_cyl_ctx steps_cyl_ctx;   /* opaque; created by init, freed by destroy */
 
 /* Plain-old-data parameter block (the quantities the problem statement
@@ -82,7 +88,7 @@ typedef struct {
                                background == STEPS_BG_FINITE                                          */
     double  rho0;           /* comoving mean density of Eq. 9/10; 0 disables the background term      */
     int32_t device;         /* CUDA device ordinal                                                    */
-    int32_t reserved;       /* must be 0                                                              */
+    int32_t flags;          /* bitwise OR of STEPS_FLAG_*; 0 = defaults                               */
 } steps_cyl_params;
 
 /* Validate `p`, select the device, allocate scratch for n particles and build the constant

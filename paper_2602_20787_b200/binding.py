@@ -16,6 +16,7 @@ STEPS_OK, STEPS_EINVAL, STEPS_ESOFT, STEPS_ECUDA, STEPS_ENOMEM, STEPS_EUNSUPPORT
 PERIODIC_IMAGES, PERIODIC_EWALD_TABLE = 0, 1
 PREC_FP64, PREC_MIXED = 0, 1
 BG_FINITE, BG_INFINITE = 0, 1
+FLAG_DETERMINISTIC = 1
 
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",
            "steps_cyl_check", "steps_cyl_background", "steps_cyl_kdk_step",
@@ -29,7 +30,7 @@ class Params(C.Structure):
     _fields_ = [("n", C.c_int64), ("Lz", C.c_double), ("G", C.c_double),
                 ("periodic_mode", C.c_int32), ("n_cut", C.c_int32), ("precision", C.c_int32),
                 ("background", C.c_int32), ("R_sim", C.c_double), ("rho0", C.c_double),
-                ("device", C.c_int32), ("reserved", C.c_int32)]
+                ("device", C.c_int32), ("flags", C.c_int32)]
 
 
 class StepsError(RuntimeError):
@@ -120,11 +121,11 @@ class StepsCyl:
     """One steps_cyl_ctx.  Methods mirror the C entry points one to one."""
 
     def __init__(self, n, Lz, G=1.0, n_cut=5, precision=PREC_FP64, background=BG_FINITE,
-                 R_sim=0.0, rho0=0.0, device=0, periodic_mode=PERIODIC_IMAGES):
+                 R_sim=0.0, rho0=0.0, device=0, periodic_mode=PERIODIC_IMAGES, flags=0):
         self._ctx = C.c_void_p()
         self.params = Params(n=int(n), Lz=float(Lz), G=float(G), periodic_mode=int(periodic_mode),
                              n_cut=int(n_cut), precision=int(precision), background=int(background),
-                             R_sim=float(R_sim), rho0=float(rho0), device=int(device), reserved=0)
+                             R_sim=float(R_sim), rho0=float(rho0), device=int(device), flags=int(flags))
         self.n = int(n)
         rc = lib().steps_cyl_init(C.byref(self.params), C.byref(self._ctx))
         if rc:

@@ -67,12 +67,18 @@ __global__ void pack_kernel(const double *__restrict__ x, const double *__restri
 }
 
 // a5: g = -G (A_x, A_y, A_z1 - L A_z2), partial sums added over source chunks in fixed order.
-__global__ void finalize_kernel(const double *__restrict__ part, int n, int n_pad, int n_chunks,
-                                double G, double L, double *__restrict__ gx,
-                                double *__restrict__ gy, double *__restrict__ gz)
+// n_chunks_fast: chunks written by the fast-path kernel that ran (1 for the symmetric kernel);
+// n_chunks_general: chunks of the general kernel, which ran instead iff 2 max(h) > L/2.
+__global__ void finalize_kernel(const double *__restrict__ part, int n, int n_pad,
+                                int n_chunks_fast, int n_chunks_general, double halfL,
+                                const DevFlags *__restrict__ flags, double G, double L,
+                                double *__restrict__ gx, double *__restrict__ gy,
+                                double *__restrict__ gz)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    const double hmax = __longlong_as_double((long long)flags->hmax_bits);
+    const int n_chunks = ((2.0 * hmax > halfL) || flags->bad_h) ? n_chunks_general : n_chunks_fast;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     for (int c = 0; c < n_chunks; ++c) {
         const double *p = part + (size_t)c * 4 * n_pad + i;

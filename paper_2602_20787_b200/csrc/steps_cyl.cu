@@ -13,6 +13,7 @@
 
 #include "aux_kernels.cuh"
 #include "pair_fp64.cuh"
+#include "pair_fp64_sym.cuh"
 #include "pair_mixed.cuh"
 
 using namespace steps;
@@ -21,6 +22,8 @@ struct steps_cyl_ctx {
     steps_cyl_params p;
     int n, n_pad, n_tiles;
     int n_chunks, tiles_per_chunk;
+    int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
+    bool use_sym;                                 // fp64 && !STEPS_FLAG_DETERMINISTIC
     int sm_count;
     PairConsts kc;
     MixedConsts mc;
@@ -95,6 +98,13 @@ void choose_chunks(steps_cyl_ctx *c)
     chunks = std::min(chunks, 64);
     c->tiles_per_chunk = (c->n_tiles + chunks - 1) / chunks;
     c->n_chunks = (c->n_tiles + c->tiles_per_chunk - 1) / c->tiles_per_chunk;
+    // symmetric kernel: CTAs cover the upper triangle of (target block, source tile); aim at
+    // >= 8 waves of non-empty CTAs, at most 64 tiles (~2 ms) per CTA.
+    const double tri = 0.5 * (double)c->n_tiles * (double)(c->n_tiles + 1);
+    int tpc = (int)(tri / (8.0 * 4.0 * c->sm_count));
+    tpc = std::max(1, std::min(tpc, 64));
+    c->sym_tiles_per_chunk = tpc;
+    c->sym_chunks = (c->n_tiles + tpc - 1) / tpc;
 }
 
 template <int NC>
@@ -104,6 +114,15 @@ void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
     pair_fp64_kernel<NC, 0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
                                                          c->tiles_per_chunk, c->p.n_cut, c->kc,
                                                          c->flags, c->part);
+}
+
+template <int NC>
+void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    dim3 grid(c->n_tiles, c->sym_chunks);
+    pair_fp64_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad,
+                                                          c->n_tiles, c->sym_tiles_per_chunk,
+                                                          c->p.n_cut, c->kc, c->flags, c->part);
 }
 
 template <int NC>
@@ -122,12 +141,14 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 #define CASE_NC(N)                                               \
     case N:                                                      \
         if (mixed) launch_pair_mixed_nc<N>(c, s);                \
+        else if (c->use_sym) launch_pair_sym_nc<N>(c, s);        \
         else launch_pair_fp64_nc<N>(c, s);                       \
         break;
         CASE_NC(1) CASE_NC(2) CASE_NC(3) CASE_NC(4) CASE_NC(5) CASE_NC(6) CASE_NC(7) CASE_NC(8)
 #undef CASE_NC
     default:
         if (mixed) launch_pair_mixed_nc<0>(c, s);
+        else if (c->use_sym) launch_pair_sym_nc<0>(c, s);
         else launch_pair_fp64_nc<0>(c, s);
     }
     // general path: a no-op unless 2 max(h) > L/2
@@ -149,11 +170,15 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
                                                      ctx->tile_hmax, ctx->flags);
     ctx->launches += 1;
     CK(cudaEventRecord(ctx->ev0, s));
+    if (ctx->use_sym)      // the symmetric kernel accumulates with atomics into part[0..4 n_pad)
+        CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * sizeof(double), s));
     launch_pair(ctx, s);
     CK(cudaEventRecord(ctx->ev1, s));
     ctx->ev_valid = true;
     finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
-                                                         ctx->n_chunks, ctx->p.G, ctx->p.Lz, gx, gy, gz);
+                                                         ctx->use_sym ? 1 : ctx->n_chunks,
+                                                         ctx->n_chunks, ctx->kc.halfL, ctx->flags,
+                                                         ctx->p.G, ctx->p.Lz, gx, gy, gz);
     ctx->launches += 1;
     CK(cudaGetLastError());
     return STEPS_OK;
@@ -186,7 +211,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     if (p->periodic_mode != STEPS_PERIODIC_IMAGES) return STEPS_EINVAL;
     if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
     if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
-    if (p->reserved != 0 || p->device < 0) return STEPS_EINVAL;
+    if ((p->flags & ~STEPS_FLAG_DETERMINISTIC) != 0 || p->device < 0) return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
     if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
 
@@ -208,6 +233,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->n_tiles = (ctx->n + PAIR_THREADS - 1) / PAIR_THREADS;
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
+    ctx->use_sym = p->precision == STEPS_PREC_FP64 && !(p->flags & STEPS_FLAG_DETERMINISTIC);
 
     const double L = p->Lz;
     ctx->kc.L = L;

@@ -24,11 +24,11 @@ def torch_cuda():
     return torch
 
 
-def gpu_accel(torch, w_arrays, Lz, G, n_cut, precision=0, host=False):
+def gpu_accel(torch, w_arrays, Lz, G, n_cut, precision=0, host=False, flags=0):
     from paper_2602_20787_b200 import binding as b
     x, y, z, m, h = [np.ascontiguousarray(a, dtype=np.float64) for a in w_arrays]
     n = x.shape[0]
-    ctx = b.StepsCyl(n=n, Lz=Lz, G=G, n_cut=n_cut, precision=precision)
+    ctx = b.StepsCyl(n=n, Lz=Lz, G=G, n_cut=n_cut, precision=precision, flags=flags)
     try:
         if host:
             out = [np.empty(n) for _ in range(3)]
@@ -200,3 +200,22 @@ def test_bench_size_sampled_targets(torch_cuda, oracle, precision):
     # momentum conservation over ALL particles (holds at any size)
     for c in g:
         assert abs(np.sum(w.m * c)) <= (1e-11 if precision == 0 else 1e-5) * np.sum(w.m * np.abs(c))
+
+
+@pytest.mark.parametrize("n", [2, 129, 700, 5000])
+def test_deterministic_ordered_kernel(torch_cuda, oracle, n):
+    """STEPS_FLAG_DETERMINISTIC: the ordered-pair kernel with fixed-order reduction -- same parity
+    bar, and bit-identical results from run to run."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(1, n=n, seed=21)
+    arrs = (w.x, w.y, w.z, w.m, w.h)
+    ref = oracle.accel(*arrs, w.Lz, w.G, 5)
+    g1 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_DETERMINISTIC)
+    g2 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_DETERMINISTIC)
+    check(g1, ref, 0)
+    for a, c in zip(g1, g2):
+        assert np.array_equal(a, c)
+    # the default (symmetric, atomics) kernel agrees with it to round-off
+    g3 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0)
+    assert rel_err(g3, g1).max() < 1e-12
