@@ -31,23 +31,40 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# FP64-pipe instruction mix of pair_fp64_kernel<5,0>, one (i, j) pair = 10 image terms, counted in
-# the SASS of the shipped kernel: 49 DFMA + 33 DMUL + 24 DADD + 3 DSETP.
-FP64_MIX = {5: dict(dfma=49, dmul=33, dadd=24, dsetp=3)}
+# Instruction mix of the pair kernels' inner loops at N_cut = 5 (10 image terms per pair), counted
+# in the SASS of the shipped library (cuobjdump -sass).  "unit" says what one
+# loop iteration covers: the symmetric kernel evaluates an UNORDERED pair (two interactions).
+KERNEL_MIX = {
+    # default fp64 kernel, pair_fp64_sym_kernel<5>: one unordered pair per iteration
+    "fp64": dict(kernel="pair_fp64_sym_kernel<5>", interactions=2, dfma=53, dmul=33, dadd=22, dsetp=0,
+                 per_image=(9.5, 14.0)),
+    # STEPS_FLAG_DETERMINISTIC, pair_fp64_kernel<5,0>: one ordered pair per iteration
+    "fp64_det": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
+                     per_image=(9.5, 14.0)),
+    # pair_mixed_kernel<5>: one ordered pair per iteration; FP32-pipe instructions + 10 MUFU.RSQ
+    "mixed": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
+                  f2f=4, dadd=4),
+}
 METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
 NOMINAL_FP64_LANES_PER_SM = 64
+NOMINAL_FP32_LANES_PER_SM = 128
+NOMINAL_XU_LANES_PER_SM = 16
 
 
-def pipe_counts(n_cut):
-    """(FP64-pipe instructions, flops) per ordered pair; n_cut != 5 scales the per-image part."""
-    mix = FP64_MIX[5]
-    instr5 = sum(mix.values())
-    flops5 = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
-    if n_cut == 5:
-        return instr5, flops5
-    per_img_i, per_img_f = 9.5, 14.0                     # far image: 9.5 instr (5 FMA) / 14 flops
-    d = 2 * (n_cut - 5)
-    return instr5 + per_img_i * d, flops5 + per_img_f * d
+def pipe_counts(mode, n_cut):
+    """(pipe instructions, flops) per ORDERED pair interaction for the kernel of `mode`."""
+    mix = KERNEL_MIX[mode]
+    if mode == "mixed":
+        instr = mix["ffma"] + mix["fmul"] + mix["fadd"]
+        flops = 2 * mix["ffma"] + mix["fmul"] + mix["fadd"]
+        d = 2 * (n_cut - 5)
+        return instr + 11.0 * d, flops + 14.0 * d
+    instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
+    flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
+    d = 2 * (n_cut - 5)                                  # extra image terms per pair evaluation
+    instr += mix["per_image"][0] * d
+    flops += mix["per_image"][1] * d
+    return instr / mix["interactions"], flops / mix["interactions"]
 
 
 class ClockSampler:
@@ -199,7 +216,8 @@ def run_ours(args):
     w = workloads.make(3, n=args.n, seed=3 + rank)
     n = w.n
     ctx = b.StepsCyl(n=n, Lz=w.Lz, G=w.G, n_cut=args.n_cut, precision=prec, background=b.BG_FINITE,
-                     R_sim=w.R_sim, rho0=w.rho0, device=local)
+                     R_sim=w.R_sim, rho0=w.rho0, device=local,
+                     flags=b.FLAG_DETERMINISTIC if args.deterministic else 0)
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
             for k in names}
@@ -261,23 +279,31 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peaks_kind = load_peaks()
-    instr, flops = pipe_counts(args.n_cut)
+    mode = "mixed" if prec == b.PREC_MIXED else ("fp64_det" if args.deterministic else "fp64")
+    instr, flops = pipe_counts(mode, args.n_cut)
     t_pair = float(np.mean(pair_ms)) * 1e-3
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    nominal_tflops = sm_count * NOMINAL_FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    lanes = NOMINAL_FP32_LANES_PER_SM if mode == "mixed" else NOMINAL_FP64_LANES_PER_SM
+    nominal_tflops = sm_count * lanes * 2 * sm_max * 1e6 / 1e12
     achieved_tflops = flops * pairs_per_step / t_pair / 1e12
     roofline = {
-        "bound": "alu", "kernel": "pair_%s_kernel<%d>" % (args.precision, args.n_cut),
+        "bound": "alu", "kernel": KERNEL_MIX[mode]["kernel"].replace("<5", "<%d" % args.n_cut),
         "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
         "frac": achieved_tflops / nominal_tflops, "traffic": None,
-        "peak_kind": "nominal FP64 FMA: %d SMs x 64 lanes x 2 flop x %.0f MHz (DESIGN.md)" % (sm_count, sm_max),
-        "flops_per_pair": flops, "fp64_pipe_instr_per_pair": instr,
-        "measured_dfma_tflops": 2 * dfma_per_s / 1e12,
-        "fp64_pipe_util_vs_measured_dfma": instr * pairs_per_step / t_pair / dfma_per_s,
-        "fp64_pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
+        "peak_kind": "nominal %s FMA: %d SMs x %d lanes x 2 flop x %.0f MHz (DESIGN.md)"
+                     % ("FP32" if mode == "mixed" else "FP64", sm_count, lanes, sm_max),
+        "flops_per_pair_interaction": flops, "pipe_instr_per_pair_interaction": instr,
+        "pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
         "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
     }
+    if mode == "mixed":
+        xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
+        mufu = 2 * args.n_cut + KERNEL_MIX["mixed"]["f2f"]
+        roofline["xu_pipe_util_vs_nominal"] = mufu * pairs_per_step / t_pair / xu_peak
+    else:
+        roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
+        roofline["pipe_util_vs_measured_dfma"] = instr * pairs_per_step / t_pair / dfma_per_s
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -324,6 +350,8 @@ def main():
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per sample / reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--deterministic", action="store_true",
+                    help="fp64: ordered-pair kernel with fixed-order reduction (STEPS_FLAG_DETERMINISTIC)")
     args = ap.parse_args()
     if args.warmup < 3:
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
