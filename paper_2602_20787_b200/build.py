@@ -29,9 +29,13 @@ def nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+def _extra() -> list:
+    return os.environ.get("STEPS_NVCC_EXTRA", "").split()
+
+
 def _source_hash() -> str:
     import hashlib
-    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    h = hashlib.sha256(" ".join(NVCC_FLAGS + _extra()).encode())
     for d in DEPS:
         h.update(open(d, "rb").read())
     return h.hexdigest()
@@ -45,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == want:
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", tmp]
+    cmd = [nvcc(), *NVCC_FLAGS, *_extra(), *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", tmp]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     with open(stamp, "w") as f:

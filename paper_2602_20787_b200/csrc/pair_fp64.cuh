@@ -127,6 +127,7 @@ __device__ __forceinline__ void image_sum(double rz, double q, double hi, double
         we = rz_nonzero ? we : 0.0;
         S += we;
         T = (NC == 1) ? copysign(we, rz) : fma(copysign((double)NC, rz), we, T);
+
     } else {
         for (int n = 1; n < ncut_rt; ++n) {
             const double nL = (double)n * k.L;

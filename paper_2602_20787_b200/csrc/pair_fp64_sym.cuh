@@ -13,7 +13,7 @@
 // registers) and walks a 32-source sub-tile as a ring: at step s lane l meets source
 // (l + s) mod 32, whose data it reads from the shared-memory tile and whose accumulator is in
 // lane l's registers; after the step the four source accumulators move one lane down
-// (8 SHFL), so that after 32 steps every accumulator is back in its home lane and has met all
+// (6 SHFL), so that after 32 steps every accumulator is back in its home lane and has met all
 // 32 targets.  Home accumulators go to a per-warp shared slab, the four slabs of the CTA are
 // summed at the end of the tile and leave with one RED.ADD.F64 per value.
 //
@@ -32,21 +32,34 @@
 
 namespace steps {
 
+#ifndef STEPS_SYM_UNROLL
+#define STEPS_SYM_UNROLL 1
+#endif
+constexpr int kSymUnroll = STEPS_SYM_UNROLL;
+#ifndef STEPS_SYM_MINBLOCKS
+#define STEPS_SYM_MINBLOCKS 4      // resident CTAs per SM the register allocation aims at
+#endif
+
+// One staged source: 48 bytes, read with two LDS.128 and one LDS.64 off a single address.
+struct __align__(16) SymSrc { double x, y, z, m, h, pad; };
+
 // 32 ring steps of one warp against one 32-source sub-tile.  SYM: also accumulate on the sources.
+// Source-side accumulators (rotating): bx = sum m_i S r_x, by = sum m_i S r_y,
+// bz = sum m_i (S r_z - L T) -- z already combined, so only three values travel.
 template <int NC, bool SYM>
 __device__ __forceinline__ void ring_subtile(double xi, double yi, double zi, double hi, double mi,
-                                             const double2 *s_xy, const double2 *s_zm,
-                                             const double *s_h, int jbase, int lane, int soft_hi,
-                                             const PairConsts &k, int ncut_rt,
+                                             double mLi, const SymSrc *s_src, int lane,
+                                             int soft_hi, const PairConsts &k, int ncut_rt,
                                              double &ax, double &ay, double &az1, double &az2,
-                                             double &bx, double &by, double &bz1, double &bz2)
+                                             double &bx, double &by, double &bz)
 {
-    bx = by = bz1 = bz2 = 0.0;
-#pragma unroll 1
+    bx = by = bz = 0.0;
+#pragma unroll kSymUnroll
     for (int s = 0; s < 32; ++s) {
-        const int jj = jbase + ((lane + s) & 31);
-        const double2 a = s_xy[jj], b = s_zm[jj];
-        const double hj = s_h[jj];
+        const SymSrc *sj = s_src + ((lane + s) & 31);
+        const double2 a = *reinterpret_cast<const double2 *>(&sj->x);
+        const double2 b = *reinterpret_cast<const double2 *>(&sj->z);
+        const double hj = sj->h;
         const double rx = xi - a.x, ry = yi - a.y;
         const double rz = nearest_image(zi - b.x, k);
         const double rho2 = fma(ry, ry, rx * rx);
@@ -60,23 +73,22 @@ __device__ __forceinline__ void ring_subtile(double xi, double yi, double zi, do
         az2 = fma(b.y, T, az2);
         if (SYM) {
             const double Si = mi * S;
-            bx  = fma(Si, rx, bx);
-            by  = fma(Si, ry, by);
-            bz1 = fma(Si, rz, bz1);
-            bz2 = fma(mi, T, bz2);
+            bx = fma(Si, rx, bx);
+            by = fma(Si, ry, by);
+            bz = fma(Si, rz, bz);
+            bz = fma(mLi, T, bz);                       // mLi = -L m_i
             const int src = (lane + 1) & 31;
-            bx  = __shfl_sync(0xffffffffu, bx, src);
-            by  = __shfl_sync(0xffffffffu, by, src);
-            bz1 = __shfl_sync(0xffffffffu, bz1, src);
-            bz2 = __shfl_sync(0xffffffffu, bz2, src);
+            bx = __shfl_sync(0xffffffffu, bx, src);
+            by = __shfl_sync(0xffffffffu, by, src);
+            bz = __shfl_sync(0xffffffffu, bz, src);
         }
     }
 }
 
 // acc layout: acc[comp * n_pad + particle], comp = 0..3 (A_x, A_y, A_z1, A_z2), zeroed by the host
-// before the launch.  grid = (n_tiles, n_chunks_sym).
+// before the launch; the source side adds its combined z sum to A_z1.  grid = (n_tiles, chunks).
 template <int NC>
-__global__ void __launch_bounds__(PAIR_THREADS, 4)
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                      const double *__restrict__ hs, const double *__restrict__ tile_hmax,
                      int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
@@ -90,23 +102,25 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
         const double hmax = __longlong_as_double((long long)flags->hmax_bits);
         if ((2.0 * hmax > k.halfL) || flags->bad_h) return;      // general kernel's job
     }
-    __shared__ double2 s_xy[PAIR_THREADS];
-    __shared__ double2 s_zm[PAIR_THREADS];
-    __shared__ double  s_h[PAIR_THREADS];
-    __shared__ double  s_b[PAIR_THREADS / 32][4][PAIR_THREADS];   // per-warp source accumulators
+    __shared__ SymSrc s_src[PAIR_THREADS];
+    __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];    // per-warp source accumulators
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int i = bi * PAIR_THREADS + threadIdx.x;
     const double2 pi = xy[i], qi = zm[i];
     const double xi = pi.x, yi = pi.y, zi = qi.x, mi = qi.y, hi = hs[i];
+    const double mLi = -k.L * mi;
     double ax = 0.0, ay = 0.0, az1 = 0.0, az2 = 0.0;
 
     for (int t = t0; t < t1; ++t) {
         const int j = t * PAIR_THREADS + threadIdx.x;
         __syncthreads();                                   // previous tile's flush has read s_b
-        s_xy[threadIdx.x] = xy[j];
-        s_zm[threadIdx.x] = zm[j];
-        s_h[threadIdx.x]  = hs[j];
+        {
+            const double2 pj = xy[j], qj = zm[j];
+            SymSrc v;
+            v.x = pj.x; v.y = pj.y; v.z = qj.x; v.m = qj.y; v.h = hs[j]; v.pad = 0.0;
+            s_src[threadIdx.x] = v;
+        }
         __syncthreads();
         int soft_hi;
         {
@@ -116,28 +130,25 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
         const bool diag = (t == bi);
 #pragma unroll 1
         for (int js = 0; js < PAIR_THREADS / 32; ++js) {
-            double bx = 0.0, by = 0.0, bz1 = 0.0, bz2 = 0.0;
+            double bx = 0.0, by = 0.0, bz = 0.0;
             if (!diag || js > w)
-                ring_subtile<NC, true>(xi, yi, zi, hi, mi, s_xy, s_zm, s_h, js * 32, lane, soft_hi,
-                                       k, ncut_rt, ax, ay, az1, az2, bx, by, bz1, bz2);
+                ring_subtile<NC, true>(xi, yi, zi, hi, mi, mLi, s_src + js * 32, lane, soft_hi, k,
+                                       ncut_rt, ax, ay, az1, az2, bx, by, bz);
             else if (js == w)
-                ring_subtile<NC, false>(xi, yi, zi, hi, mi, s_xy, s_zm, s_h, js * 32, lane, soft_hi,
-                                        k, ncut_rt, ax, ay, az1, az2, bx, by, bz1, bz2);
+                ring_subtile<NC, false>(xi, yi, zi, hi, mi, mLi, s_src + js * 32, lane, soft_hi, k,
+                                        ncut_rt, ax, ay, az1, az2, bx, by, bz);
             const int jl = js * 32 + lane;
             s_b[w][0][jl] = bx;
             s_b[w][1][jl] = by;
-            s_b[w][2][jl] = bz1;
-            s_b[w][3][jl] = bz2;
+            s_b[w][2][jl] = bz;
         }
         __syncthreads();
-        {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                double v = s_b[0][c][threadIdx.x];
+        for (int c = 0; c < 3; ++c) {
+            double v = s_b[0][c][threadIdx.x];
 #pragma unroll
-                for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
-                if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
-            }
+            for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
+            if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
         }
     }
     atomicAdd(acc + i, ax);
