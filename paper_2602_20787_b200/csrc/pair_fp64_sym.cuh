@@ -43,40 +43,49 @@ constexpr int kSymUnroll = STEPS_SYM_UNROLL;
 // One staged source: 48 bytes, read with two LDS.128 and one LDS.64 off a single address.
 struct __align__(16) SymSrc { double x, y, z, m, h, pad; };
 
-// 32 ring steps of one warp against one 32-source sub-tile.  SYM: also accumulate on the sources.
-// Source-side accumulators (rotating): bx = sum m_i S r_x, by = sum m_i S r_y,
-// bz = sum m_i (S r_z - L T) -- z already combined, so only three values travel.
-template <int NC, bool SYM>
-__device__ __forceinline__ void ring_subtile(double xi, double yi, double zi, double hi, double mi,
-                                             double mLi, const SymSrc *s_src, int lane,
-                                             int soft_hi, const PairConsts &k, int ncut_rt,
-                                             double &ax, double &ay, double &az1, double &az2,
-                                             double &bx, double &by, double &bz)
+// Targets a lane keeps in registers (R = SYM_R of them, one per target tile of the CTA).
+struct SymTgt { double x, y, z, h, m, mL; };         // mL = -L m
+
+// 32 ring steps of one warp against one 32-source sub-tile.  R targets per lane meet the same
+// source in a step, so the source record is loaded and its accumulators are shuffled once per R
+// pairs.  SYM: also accumulate on the sources.  Source-side accumulators (rotating):
+// bx = sum m_i S r_x, by = sum m_i S r_y, bz = sum m_i (S r_z - L T) -- z already combined,
+// so only three values travel.
+template <int NC, int R, bool SYM>
+__device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&soft_hi)[R],
+                                             const SymSrc *s_src, int lane, const PairConsts &k,
+                                             int ncut_rt, double (&a)[R][4], double &bx,
+                                             double &by, double &bz)
 {
     bx = by = bz = 0.0;
 #pragma unroll kSymUnroll
     for (int s = 0; s < 32; ++s) {
         const SymSrc *sj = s_src + ((lane + s) & 31);
-        const double2 a = *reinterpret_cast<const double2 *>(&sj->x);
-        const double2 b = *reinterpret_cast<const double2 *>(&sj->z);
+        const double2 pa = *reinterpret_cast<const double2 *>(&sj->x);
+        const double2 pb = *reinterpret_cast<const double2 *>(&sj->z);
         const double hj = sj->h;
-        const double rx = xi - a.x, ry = yi - a.y;
-        const double rz = nearest_image(zi - b.x, k);
-        const double rho2 = fma(ry, ry, rx * rx);
-        const double q = fma(rz, rz, rho2);
-        double S, T;
-        image_sum<NC>(rz, q, hi, hj, soft_hi, k, ncut_rt, S, T);
-        const double Sj = b.y * S;
-        ax  = fma(Sj, rx, ax);
-        ay  = fma(Sj, ry, ay);
-        az1 = fma(Sj, rz, az1);
-        az2 = fma(b.y, T, az2);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
+            const double rz = nearest_image(ti[r].z - pb.x, k);
+            const double rho2 = fma(ry, ry, rx * rx);
+            const double q = fma(rz, rz, rho2);
+            double S, T;
+            image_sum<NC>(rz, q, ti[r].h, hj, soft_hi[r], k, ncut_rt, S, T);
+            const double Sj = pb.y * S;
+            a[r][0] = fma(Sj, rx, a[r][0]);
+            a[r][1] = fma(Sj, ry, a[r][1]);
+            a[r][2] = fma(Sj, rz, a[r][2]);
+            a[r][3] = fma(pb.y, T, a[r][3]);
+            if (SYM) {
+                const double Si = ti[r].m * S;
+                bx = fma(Si, rx, bx);
+                by = fma(Si, ry, by);
+                bz = fma(Si, rz, bz);
+                bz = fma(ti[r].mL, T, bz);
+            }
+        }
         if (SYM) {
-            const double Si = mi * S;
-            bx = fma(Si, rx, bx);
-            by = fma(Si, ry, by);
-            bz = fma(Si, rz, bz);
-            bz = fma(mLi, T, bz);                       // mLi = -L m_i
             const int src = (lane + 1) & 31;
             bx = __shfl_sync(0xffffffffu, bx, src);
             by = __shfl_sync(0xffffffffu, by, src);
@@ -85,8 +94,15 @@ __device__ __forceinline__ void ring_subtile(double xi, double yi, double zi, do
     }
 }
 
+#ifndef STEPS_SYM_R
+#define STEPS_SYM_R 2
+#endif
+constexpr int SYM_R = STEPS_SYM_R;     // target tiles per CTA (n_tiles is kept a multiple of SYM_R by the host)
+
 // acc layout: acc[comp * n_pad + particle], comp = 0..3 (A_x, A_y, A_z1, A_z2), zeroed by the host
-// before the launch; the source side adds its combined z sum to A_z1.  grid = (n_tiles, chunks).
+// before the launch; the source side adds its combined z sum to A_z1.
+// grid = (n_tiles / SYM_R, chunks).  CTA (bi, c): target tiles SYM_R*bi + r (lane holds particle
+// tid of each), source tiles [c*tpc, (c+1)*tpc) from SYM_R*bi on.
 template <int NC>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
@@ -94,8 +110,8 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
                      int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
                      const DevFlags *__restrict__ flags, double *__restrict__ acc)
 {
-    const int bi = blockIdx.x;
-    const int t0 = max(blockIdx.y * tiles_per_chunk, bi);
+    const int tb = blockIdx.x * SYM_R;                       // first target tile of this CTA
+    const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
     {
@@ -106,11 +122,16 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
     __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];    // per-warp source accumulators
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int i = bi * PAIR_THREADS + threadIdx.x;
-    const double2 pi = xy[i], qi = zm[i];
-    const double xi = pi.x, yi = pi.y, zi = qi.x, mi = qi.y, hi = hs[i];
-    const double mLi = -k.L * mi;
-    double ax = 0.0, ay = 0.0, az1 = 0.0, az2 = 0.0;
+    SymTgt ti[SYM_R];
+    double a[SYM_R][4];
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+        const double2 pi = xy[i], qi = zm[i];
+        ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
+        ti[r].mL = -k.L * qi.y;
+        a[r][0] = a[r][1] = a[r][2] = a[r][3] = 0.0;
+    }
 
     for (int t = t0; t < t1; ++t) {
         const int j = t * PAIR_THREADS + threadIdx.x;
@@ -122,21 +143,40 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             s_src[threadIdx.x] = v;
         }
         __syncthreads();
-        int soft_hi;
+        int soft_hi[SYM_R];
         {
-            const double b = hi + tile_hmax[t];
-            soft_hi = hi32(b * b);
+            const double hm = tile_hmax[t];
+#pragma unroll
+            for (int r = 0; r < SYM_R; ++r) {
+                const double b = ti[r].h + hm;
+                soft_hi[r] = hi32(b * b);
+            }
         }
-        const bool diag = (t == bi);
 #pragma unroll 1
         for (int js = 0; js < PAIR_THREADS / 32; ++js) {
             double bx = 0.0, by = 0.0, bz = 0.0;
-            if (!diag || js > w)
-                ring_subtile<NC, true>(xi, yi, zi, hi, mi, mLi, s_src + js * 32, lane, soft_hi, k,
-                                       ncut_rt, ax, ay, az1, az2, bx, by, bz);
-            else if (js == w)
-                ring_subtile<NC, false>(xi, yi, zi, hi, mi, mLi, s_src + js * 32, lane, soft_hi, k,
-                                        ncut_rt, ax, ay, az1, az2, bx, by, bz);
+            const SymSrc *sub = s_src + js * 32;
+            if (t >= tb + SYM_R) {
+                // off-diagonal tile: every target of the CTA meets every source, both ways
+                ring_subtile<NC, SYM_R, true>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+            } else {
+                // one of the CTA's own tiles: target tile tb + r meets source tile t only if
+                // t >= tb + r; in its own tile (t == tb + r) warp w takes sub-tiles js > w both
+                // ways, js == w target-side only, and leaves js < w to the warp that owns them.
+#pragma unroll
+                for (int r = 0; r < SYM_R; ++r) {
+                    if (tb + r > t) continue;
+                    const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
+                    const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
+                    double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
+                    double cx = 0.0, cy = 0.0, cz = 0.0;
+                    if (tb + r < t || js > w)
+                        ring_subtile<NC, 1, true>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                    else if (js == w)
+                        ring_subtile<NC, 1, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                    bx += cx; by += cy; bz += cz;
+                }
+            }
             const int jl = js * 32 + lane;
             s_b[w][0][jl] = bx;
             s_b[w][1][jl] = by;
@@ -151,10 +191,12 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
         }
     }
-    atomicAdd(acc + i, ax);
-    atomicAdd(acc + (size_t)n_pad + i, ay);
-    atomicAdd(acc + 2 * (size_t)n_pad + i, az1);
-    atomicAdd(acc + 3 * (size_t)n_pad + i, az2);
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
+    }
 }
 
 }  // namespace steps

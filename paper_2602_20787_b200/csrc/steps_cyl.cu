@@ -119,7 +119,7 @@ void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
 template <int NC>
 void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
-    dim3 grid(c->n_tiles, c->sym_chunks);
+    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
     pair_fp64_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad,
                                                           c->n_tiles, c->sym_tiles_per_chunk,
                                                           c->p.n_cut, c->kc, c->flags, c->part);
@@ -230,7 +230,8 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->sm_count = prop.multiProcessorCount;
 
     ctx->n = (int)p->n;
-    ctx->n_tiles = (ctx->n + PAIR_THREADS - 1) / PAIR_THREADS;
+    // a multiple of SYM_R tiles: the symmetric kernel's CTAs own SYM_R target tiles each
+    ctx->n_tiles = SYM_R * ((ctx->n + SYM_R * PAIR_THREADS - 1) / (SYM_R * PAIR_THREADS));
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
     ctx->use_sym = p->precision == STEPS_PREC_FP64 && !(p->flags & STEPS_FLAG_DETERMINISTIC);
