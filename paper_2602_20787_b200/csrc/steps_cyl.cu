@@ -15,6 +15,7 @@
 #include "pair_fp64.cuh"
 #include "pair_fp64_sym.cuh"
 #include "pair_mixed.cuh"
+#include "pair_mixed_sym.cuh"
 
 using namespace steps;
 
@@ -23,7 +24,7 @@ struct steps_cyl_ctx {
     int n, n_pad, n_tiles;
     int n_chunks, tiles_per_chunk;
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
-    bool use_sym;                                 // fp64 && !STEPS_FLAG_DETERMINISTIC
+    bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
     int sm_count;
     PairConsts kc;
     MixedConsts mc;
@@ -134,20 +135,32 @@ void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
                                                        c->kc.halfL, c->flags, c->part);
 }
 
+template <int NC>
+void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
+    pair_mixed_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax, c->n_pad,
+                                                           c->n_tiles, c->sym_tiles_per_chunk,
+                                                           c->p.n_cut, c->mc, c->kc.halfL, c->flags,
+                                                           c->part);
+}
+
 void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
     const bool mixed = c->p.precision == STEPS_PREC_MIXED;
     switch (c->p.n_cut) {
 #define CASE_NC(N)                                               \
     case N:                                                      \
-        if (mixed) launch_pair_mixed_nc<N>(c, s);                \
+        if (mixed && c->use_sym) launch_pair_mixed_sym_nc<N>(c, s); \
+        else if (mixed) launch_pair_mixed_nc<N>(c, s);           \
         else if (c->use_sym) launch_pair_sym_nc<N>(c, s);        \
         else launch_pair_fp64_nc<N>(c, s);                       \
         break;
         CASE_NC(1) CASE_NC(2) CASE_NC(3) CASE_NC(4) CASE_NC(5) CASE_NC(6) CASE_NC(7) CASE_NC(8)
 #undef CASE_NC
     default:
-        if (mixed) launch_pair_mixed_nc<0>(c, s);
+        if (mixed && c->use_sym) launch_pair_mixed_sym_nc<0>(c, s);
+        else if (mixed) launch_pair_mixed_nc<0>(c, s);
         else if (c->use_sym) launch_pair_sym_nc<0>(c, s);
         else launch_pair_fp64_nc<0>(c, s);
     }
@@ -234,7 +247,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->n_tiles = SYM_R * ((ctx->n + SYM_R * PAIR_THREADS - 1) / (SYM_R * PAIR_THREADS));
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
-    ctx->use_sym = p->precision == STEPS_PREC_FP64 && !(p->flags & STEPS_FLAG_DETERMINISTIC);
+    ctx->use_sym = !(p->flags & STEPS_FLAG_DETERMINISTIC);
 
     const double L = p->Lz;
     ctx->kc.L = L;
