@@ -41,9 +41,13 @@ KERNEL_MIX = {
     # STEPS_FLAG_DETERMINISTIC, pair_fp64_kernel<5,0>: one ordered pair per iteration
     "fp64_det": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
                      per_image=(9.5, 14.0)),
-    # pair_mixed_kernel<5>: one ordered pair per iteration; FP32-pipe instructions + 10 MUFU.RSQ
-    "mixed": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
-                  f2f=4, dadd=4),
+    # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
+    # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
+    "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=25, fmul=24, fadd=29, mufu=10,
+                  f2f=0, dadd=0),
+    # STEPS_FLAG_DETERMINISTIC, pair_mixed_kernel<5>: one ordered pair per iteration
+    "mixed_det": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
+                      f2f=4, dadd=4),
 }
 METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
 NOMINAL_FP64_LANES_PER_SM = 64
@@ -54,11 +58,11 @@ NOMINAL_XU_LANES_PER_SM = 16
 def pipe_counts(mode, n_cut):
     """(pipe instructions, flops) per ORDERED pair interaction for the kernel of `mode`."""
     mix = KERNEL_MIX[mode]
-    if mode == "mixed":
+    if mode.startswith("mixed"):
         instr = mix["ffma"] + mix["fmul"] + mix["fadd"]
         flops = 2 * mix["ffma"] + mix["fmul"] + mix["fadd"]
         d = 2 * (n_cut - 5)
-        return instr + 11.0 * d, flops + 14.0 * d
+        return (instr + 7.5 * d) / mix["interactions"], (flops + 9.0 * d) / mix["interactions"]
     instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
     flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
     d = 2 * (n_cut - 5)                                  # extra image terms per pair evaluation
@@ -279,12 +283,13 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peaks_kind = load_peaks()
-    mode = "mixed" if prec == b.PREC_MIXED else ("fp64_det" if args.deterministic else "fp64")
+    mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
     instr, flops = pipe_counts(mode, args.n_cut)
     t_pair = float(np.mean(pair_ms)) * 1e-3
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    lanes = NOMINAL_FP32_LANES_PER_SM if mode == "mixed" else NOMINAL_FP64_LANES_PER_SM
+    is_mixed = mode.startswith("mixed")
+    lanes = NOMINAL_FP32_LANES_PER_SM if is_mixed else NOMINAL_FP64_LANES_PER_SM
     nominal_tflops = sm_count * lanes * 2 * sm_max * 1e6 / 1e12
     achieved_tflops = flops * pairs_per_step / t_pair / 1e12
     roofline = {
@@ -292,14 +297,14 @@ def run_ours(args):
         "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
         "frac": achieved_tflops / nominal_tflops, "traffic": None,
         "peak_kind": "nominal %s FMA: %d SMs x %d lanes x 2 flop x %.0f MHz (DESIGN.md)"
-                     % ("FP32" if mode == "mixed" else "FP64", sm_count, lanes, sm_max),
+                     % ("FP32" if is_mixed else "FP64", sm_count, lanes, sm_max),
         "flops_per_pair_interaction": flops, "pipe_instr_per_pair_interaction": instr,
         "pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
         "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
     }
-    if mode == "mixed":
+    if is_mixed:
         xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
-        mufu = 2 * args.n_cut + KERNEL_MIX["mixed"]["f2f"]
+        mufu = (2 * args.n_cut + KERNEL_MIX[mode]["f2f"]) / KERNEL_MIX[mode]["interactions"]
         roofline["xu_pipe_util_vs_nominal"] = mufu * pairs_per_step / t_pair / xu_peak
     else:
         roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
@@ -318,7 +323,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64" if prec == b.PREC_FP64 else "f32 pair terms / f64 accumulate",
+        "dtype": "f64" if prec == b.PREC_FP64 else "f32",
         "data": "synthetic",
         "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving KDK step (Om=0.3, OL=0.7, "
                                "a 0.02->0.025), L=100 Mpc/h, r_max=1000, n_cut=%d (10 images/pair), "
