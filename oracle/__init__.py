@@ -67,6 +67,17 @@ def lib():
         _lib.oracle_friedmann_rk4.argtypes = [d] * 7 + [p, p]
         _lib.oracle_background.restype = None
         _lib.oracle_background.argtypes = [i64, p, p, d, d, d, d, i, p, p]
+        _lib.oracle_ewald_force.restype = None
+        _lib.oracle_ewald_force.argtypes = [d, d, d, d, i, i, p]
+        _lib.oracle_ewald_D.restype = None
+        _lib.oracle_ewald_D.argtypes = [d, d, d, d, i, i, p]
+        _lib.oracle_ewald_table.restype = None
+        _lib.oracle_ewald_table.argtypes = [d, d, i, i, i, i, d, p]
+        _lib.oracle_table_interp.restype = None
+        _lib.oracle_table_interp.argtypes = [p, i, i, d, d, i, d, d, p]
+        _lib.oracle_accel_table.restype = i
+        _lib.oracle_accel_table.argtypes = [i64, p, p, p, p, p, d, d, p, i, i, d, i, i64,
+                                            C.POINTER(C.c_int64), p, p, p, i]
         _lib.oracle_kdk_step.restype = i
         _lib.oracle_kdk_step.argtypes = [i64] + [p] * 11 + [d, d, i, d, d, i, d, d, d, d, d, i]
     return _lib
@@ -155,3 +166,51 @@ def kdk_step(x, y, z, vx, vy, vz, m, h, gx, gy, gz, L, G, ncut, R, rho0, mode,
                                float(a_np1), float(H_np1), float(dt), int(nthreads))
     if rc:
         raise ValueError("oracle_kdk_step: bad arguments")
+
+
+def ewald_force(rho, z, L, alpha, nmax, mmax):
+    """Eq. 12-16 (reading G4): (F_rho, F_z) per unit G m_i m_j of the one-axis-periodic point mass."""
+    F = np.zeros(2)
+    lib().oracle_ewald_force(float(rho), float(z), float(L), float(alpha), int(nmax), int(mmax), _dp(F))
+    return F
+
+
+def ewald_D(rho, z, L, alpha, nmax, mmax):
+    """Eq. 17 at one point: Ewald force minus the unsoftened nearest-image force."""
+    F = np.zeros(2)
+    lib().oracle_ewald_D(float(rho), float(z), float(L), float(alpha), int(nmax), int(mmax), _dp(F))
+    return F
+
+
+def ewald_table(L, alpha, nmax, mmax, nrho, nz, rho_max):
+    """Eq. 17 on the (nrho x nz) grid; returns D[nrho, nz, 2]."""
+    D = np.zeros((int(nrho), int(nz), 2))
+    lib().oracle_ewald_table(float(L), float(alpha), int(nmax), int(mmax), int(nrho), int(nz),
+                             float(rho_max), _dp(D))
+    return D
+
+
+def table_interp(D, rho_max, L, interp, rho, az):
+    D = _f64(D)
+    out = np.zeros(2)
+    lib().oracle_table_interp(_dp(D), D.shape[0], D.shape[1], float(rho_max), float(L), int(interp),
+                              float(rho), float(az), _dp(out))
+    return out
+
+
+def accel_table(x, y, z, m, h, L, G, D, rho_max, interp, targets=None, nthreads=0):
+    """Pair sum in EWALD_TABLE mode: softened nearest image + interpolated D (Eq. 17)."""
+    x, y, z, m, h, D = map(_f64, (x, y, z, m, h, D))
+    n = x.shape[0]
+    if targets is None:
+        nt, tp = n, None
+    else:
+        targets = np.ascontiguousarray(targets, dtype=np.int64)
+        nt, tp = targets.shape[0], targets.ctypes.data_as(C.POINTER(C.c_int64))
+    gx, gy, gz = np.empty(nt), np.empty(nt), np.empty(nt)
+    rc = lib().oracle_accel_table(n, _dp(x), _dp(y), _dp(z), _dp(m), _dp(h), float(L), float(G),
+                                  _dp(D), D.shape[0], D.shape[1], float(rho_max), int(interp),
+                                  nt, tp, _dp(gx), _dp(gy), _dp(gz), int(nthreads))
+    if rc:
+        raise ValueError("oracle_accel_table: bad arguments")
+    return gx, gy, gz

@@ -308,3 +308,249 @@ int oracle_kdk_step(int64_t n, double *x, double *y, double *z,
     }
     return 0;
 }
+
+/* ================================================================== Sect. 2.2
+ * Ewald summation in S^1 x R^2 and the correction lookup table (Eq. 12-17).
+ * Unit source at the origin, target at radial separation rho >= 0 and axial separation z;
+ * returns the force per unit (G m_i m_j): F[0] radial (negative = towards the axis of the
+ * source), F[1] axial.
+ *
+ *   Eq. 13 (real space, as printed):
+ *     F_real = - sum_{n=-nmax}^{nmax} r_n/|r_n|^3 [ erfc(alpha |r_n|) + (2 alpha/sqrt(pi)) |r_n| exp(-alpha^2 |r_n|^2) ],
+ *     r_n = r + n L e_z
+ *   Eq. 14-15 (Fourier space) -- DESIGN.md reading G4: the printed kernel B is that of the
+ *   two-axis-periodic slab problem and does not reproduce the image sum.  For one periodic axis
+ *   the two-dimensional Fourier integral of the Gaussian-filtered Green function is
+ *     E(k, rho) = int_{1/(4 alpha^2)}^{inf} t^-1 exp(-rho^2/(4t) - k^2 t) dt   (-> 2 K_0(k rho), alpha -> inf)
+ *     F_Fourier = + (2/L) sum_{m=1}^{mmax} grad[ cos(k_m z) E(k_m, rho) ],   k_m = 2 pi m / L
+ *   Eq. 16 (m = 0 mode, as printed):  F_rho = -(2/(L rho)) (1 - exp(-alpha^2 rho^2)).
+ * The integrals over t are done numerically (composite 20-point Gauss-Legendre in u = ln(k^2 t)). */
+
+static const double GL20_X[10] = {
+    0.0765265211334973337546404, 0.2277858511416450780804962, 0.3737060887154195606725482,
+    0.5108670019508270980043641, 0.6360536807265150254528367, 0.7463319064601507926143051,
+    0.8391169718222188233945291, 0.9122344282513259058677524, 0.9639719272779137912676661,
+    0.9931285991850949247861224};
+static const double GL20_W[10] = {
+    0.1527533871307258506980843, 0.1491729864726037467878287, 0.1420961093183820513292983,
+    0.1316886384491766268984945, 0.1181945319615184173123774, 0.1019301198172404350367501,
+    0.0832767415767047487247581, 0.0626720483341090635695065, 0.0406014298003869413310400,
+    0.0176140071391521183118620};
+
+/* I_p(a, s0) = int_{s0}^{inf} s^-p exp(-a/s - s) ds,  p = 1 or 2  (s = k^2 t, a = k^2 rho^2 / 4) */
+static double ewald_Ip(int p, double a, double s0)
+{
+    /* in u = ln s:  int exp(-a e^-u - e^u) e^{(1-p) u} du; the integrand is < 1e-300 beyond
+     * s = 700; panels of width 0.25 in u */
+    double u0 = log(s0), u1 = log(s0 + 700.0 + 2.0 * sqrt(a));
+    int np = (int)ceil((u1 - u0) / 0.25);
+    double hp = (u1 - u0) / np, sum = 0.0;
+    for (int i = 0; i < np; ++i) {
+        double c = u0 + (i + 0.5) * hp, hw = 0.5 * hp;
+        for (int q = 0; q < 10; ++q) {
+            for (int sg = -1; sg <= 1; sg += 2) {
+                double u = c + sg * hw * GL20_X[q];
+                double s = exp(u);
+                sum += hw * GL20_W[q] * exp(-a / s - s + (1.0 - p) * u);
+            }
+        }
+    }
+    return sum;
+}
+
+void oracle_ewald_force(double rho, double z, double L, double alpha, int nmax, int mmax,
+                        double F[2])
+{
+    const double pi = 3.14159265358979323846, two_over_sqrtpi = 1.12837916709551257390;
+    double Fr = 0.0, Fz = 0.0;
+    /* Eq. 13 */
+    for (int n = -nmax; n <= nmax; ++n) {
+        double dz = z + (double)n * L;
+        double r = sqrt(rho * rho + dz * dz);
+        if (r == 0.0) continue;
+        double br = erfc(alpha * r) + two_over_sqrtpi * alpha * r * exp(-alpha * alpha * r * r);
+        Fr += -rho / (r * r * r) * br;
+        Fz += -dz / (r * r * r) * br;
+    }
+    /* Eq. 14-15 (reading G4) */
+    for (int m = 1; m <= mmax; ++m) {
+        double k = 2.0 * pi * (double)m / L;
+        double s0 = k * k / (4.0 * alpha * alpha), a = 0.25 * k * k * rho * rho;
+        double E = ewald_Ip(1, a, s0);
+        double dE = -0.5 * k * k * rho * ewald_Ip(2, a, s0);        /* dE/drho */
+        Fr += 2.0 / L * cos(k * z) * dE;
+        Fz += -2.0 / L * k * sin(k * z) * E;
+    }
+    /* Eq. 16 */
+    if (rho > 0.0) Fr += -2.0 / (L * rho) * (1.0 - exp(-alpha * alpha * rho * rho));
+    F[0] = Fr; F[1] = Fz;
+}
+
+/* Eq. 17: D(rho, z) = F_{S1xR2}(rho, z) - F_{R3}(rho, z) on an equally spaced grid,
+ * rho_i = i rho_max/(nrho-1), z_j = j (L/2)/(nz-1)  (reading T1: the paper gives the
+ * grid size 144 x 128, not its extent or which axis is which).  F_R3 is the unsoftened
+ * nearest-image Newtonian force -r/|r|^3.  The n = 0 term of Eq. 13 and F_R3 are combined
+ * analytically, -r/r^3 [erfc(x) + 2x/sqrt(pi) e^{-x^2} - 1] = + r/r^3 [erf(x) - 2x/sqrt(pi) e^{-x^2}],
+ * x = alpha r, with its Taylor series for small x, so that D is finite at r = 0.
+ * Layout: D[(i*nz + j)*2 + c], c = 0 radial, 1 axial. */
+static double ewald_near_factor(double alpha, double r)
+{
+    /* [erf(x) - (2/sqrt(pi)) x exp(-x^2)] / r^3 */
+    const double two_over_sqrtpi = 1.12837916709551257390;
+    double x = alpha * r;
+    if (x < 0.2) {
+        /* (2/sqrt(pi)) alpha^3 sum_{k>=1} (-1)^{k+1} 2k/((2k+1) k!) x^{2k-2} */
+        double x2 = x * x, term = 1.0, sum = 0.0, fact = 1.0;
+        for (int k = 1; k <= 12; ++k) {
+            fact *= (double)k;
+            double ck = 2.0 * k / ((2.0 * k + 1.0) * fact);
+            sum += ((k & 1) ? 1.0 : -1.0) * ck * term;
+            term *= x2;
+        }
+        return two_over_sqrtpi * alpha * alpha * alpha * sum;
+    }
+    return (erf(x) - two_over_sqrtpi * x * exp(-x * x)) / (r * r * r);
+}
+
+void oracle_ewald_D(double rho, double z, double L, double alpha, int nmax, int mmax, double D[2])
+{
+    /* full Ewald force minus nearest image, with the n = 0 real-space term replaced by the
+     * combined form above; z must lie in [-L/2, L/2] */
+    const double pi = 3.14159265358979323846, two_over_sqrtpi = 1.12837916709551257390;
+    double Fr = 0.0, Fz = 0.0;
+    double r0 = sqrt(rho * rho + z * z);
+    double nf = ewald_near_factor(alpha, r0);
+    Fr += rho * nf;
+    Fz += z * nf;
+    for (int n = -nmax; n <= nmax; ++n) {
+        if (n == 0) continue;
+        double dz = z + (double)n * L;
+        double r = sqrt(rho * rho + dz * dz);
+        double br = erfc(alpha * r) + two_over_sqrtpi * alpha * r * exp(-alpha * alpha * r * r);
+        Fr += -rho / (r * r * r) * br;
+        Fz += -dz / (r * r * r) * br;
+    }
+    for (int m = 1; m <= mmax; ++m) {
+        double k = 2.0 * pi * (double)m / L;
+        double s0 = k * k / (4.0 * alpha * alpha), a = 0.25 * k * k * rho * rho;
+        Fr += 2.0 / L * cos(k * z) * (-0.5 * k * k * rho * ewald_Ip(2, a, s0));
+        Fz += -2.0 / L * k * sin(k * z) * ewald_Ip(1, a, s0);
+    }
+    if (rho > 0.0) {
+        double x = alpha * rho;
+        /* (1 - exp(-x^2))/rho, series-safe */
+        Fr += -2.0 / L * (x < 1e-4 ? alpha * alpha * rho : -expm1(-x * x) / rho);
+    }
+    D[0] = Fr; D[1] = Fz;
+}
+
+void oracle_ewald_table(double L, double alpha, int nmax, int mmax, int nrho, int nz,
+                        double rho_max, double *D)
+{
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < nrho; ++i) {
+        double rho = rho_max * (double)i / (double)(nrho - 1);
+        for (int j = 0; j < nz; ++j) {
+            double z = 0.5 * L * (double)j / (double)(nz - 1);
+            oracle_ewald_D(rho, z, L, alpha, nmax, mmax, &D[((size_t)i * nz + j) * 2]);
+        }
+    }
+}
+
+/* Table value with the symmetries of D used as boundary rules (reading T3):
+ * D_rho is odd in rho and even in z, D_z is even in rho and odd in z; both are periodic in z,
+ * so about z = L/2 D_rho is even and D_z odd.  Beyond the last radial node the last node is
+ * used.  c = 0 radial, 1 axial. */
+static double table_get(const double *D, int nrho, int nz, int i, int j, int c)
+{
+    double sgn = 1.0;
+    if (i < 0) { i = -i; if (c == 0) sgn = -sgn; }
+    if (i > nrho - 1) i = nrho - 1;
+    if (j < 0) { j = -j; if (c == 1) sgn = -sgn; }
+    if (j > nz - 1) { j = 2 * (nz - 1) - j; if (c == 1) sgn = -sgn; }
+    return sgn * D[((size_t)i * nz + j) * 2 + c];
+}
+
+/* Interpolated D at (rho, az), az = |z| in [0, L/2]: interp 0 = cloud-in-cell (bilinear),
+ * 1 = triangular-shaped-cloud (quadratic B-spline weights on the 3x3 nearest nodes),
+ * PAPER.md:164. */
+void oracle_table_interp(const double *D, int nrho, int nz, double rho_max, double L,
+                         int interp, double rho, double az, double out[2])
+{
+    double xr = rho / (rho_max / (double)(nrho - 1));
+    double xz = az / (0.5 * L / (double)(nz - 1));
+    out[0] = out[1] = 0.0;
+    if (interp == 0) {
+        int i0 = (int)floor(xr), j0 = (int)floor(xz);
+        double fr = xr - i0, fz = xz - j0;
+        double wr[2] = {1.0 - fr, fr}, wz[2] = {1.0 - fz, fz};
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b)
+                for (int c = 0; c < 2; ++c)
+                    out[c] += wr[a] * wz[b] * table_get(D, nrho, nz, i0 + a, j0 + b, c);
+    } else {
+        int ic = (int)floor(xr + 0.5), jc = (int)floor(xz + 0.5);
+        double dr = xr - ic, dz = xz - jc;
+        double wr[3] = {0.5 * (0.5 - dr) * (0.5 - dr), 0.75 - dr * dr, 0.5 * (0.5 + dr) * (0.5 + dr)};
+        double wz[3] = {0.5 * (0.5 - dz) * (0.5 - dz), 0.75 - dz * dz, 0.5 * (0.5 + dz) * (0.5 + dz)};
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b)
+                for (int c = 0; c < 2; ++c)
+                    out[c] += wr[a] * wz[b] * table_get(D, nrho, nz, ic - 1 + a, jc - 1 + b, c);
+    }
+}
+
+/* Pair sum in EWALD_TABLE mode (Eq. 7-style use of the table):
+ *   F(r, h) = F_R3(nearest image, spline-softened, Eq. 3/4) + D(rho, z)        rho < rho_max
+ *           = -2 G/(L rho) e_rho  (the line-mass term, Eq. 16 with alpha -> inf) rho >= rho_max
+ * (reading T2: the paper does not say what happens beyond the table).
+ * D is the table built with G = 1.  Same conventions as oracle_accel. */
+int oracle_accel_table(int64_t n, const double *x, const double *y, const double *z,
+                       const double *m, const double *h, double L, double G,
+                       const double *D, int nrho, int nz, double rho_max, int interp,
+                       int64_t nt, const int64_t *targets,
+                       double *gx, double *gy, double *gz, int nthreads)
+{
+    if (n < 1 || L <= 0.0 || !D || nrho < 2 || nz < 2 || rho_max <= 0.0) return -1;
+    if (!targets) nt = n;
+    double *zw = (double *)malloc((size_t)n * sizeof(double));
+    if (!zw) return -1;
+    for (int64_t j = 0; j < n; ++j) {
+        zw[j] = z[j] - L * floor(z[j] / L);
+        if (zw[j] >= L) zw[j] -= L;
+    }
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t t = 0; t < nt; ++t) {
+        int64_t i = targets ? targets[t] : t;
+        long double acc[3] = {0.0L, 0.0L, 0.0L};
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double rx = x[i] - x[j], ry = y[i] - y[j], rz = zw[i] - zw[j];
+            rz = rz - L * rint(rz / L);
+            double rho = sqrt(rx * rx + ry * ry);
+            double f[3];
+            if (rho < rho_max) {
+                double s = sqrt(rx * rx + ry * ry + rz * rz);
+                double w = (s == 0.0) ? 0.0 : oracle_spline_F(s, h[i] + h[j]) / s;
+                double Dv[2];
+                oracle_table_interp(D, nrho, nz, rho_max, L, interp, rho, fabs(rz), Dv);
+                double dr = (rho == 0.0) ? 0.0 : Dv[0] / rho;
+                f[0] = -w * rx + dr * rx;
+                f[1] = -w * ry + dr * ry;
+                f[2] = -w * rz + (rz < 0.0 ? -Dv[1] : Dv[1]);
+            } else {
+                double c = -2.0 / (L * rho * rho);
+                f[0] = c * rx; f[1] = c * ry; f[2] = 0.0;
+            }
+            acc[0] += (long double)(G * m[j] * f[0]);
+            acc[1] += (long double)(G * m[j] * f[1]);
+            acc[2] += (long double)(G * m[j] * f[2]);
+        }
+        gx[t] = (double)acc[0]; gy[t] = (double)acc[1]; gz[t] = (double)acc[2];
+    }
+    free(zw);
+    return 0;
+}
