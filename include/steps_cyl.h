@@ -55,14 +55,18 @@ typedef enum {
     STEPS_ESOFT        = -2,  /* softening precondition violated: some h_i <= 0 (or NaN)                   */
     STEPS_ECUDA        = -3,  /* a CUDA runtime call failed (or no device present)                     */
     STEPS_ENOMEM       = -4,  /* host or device allocation failed                                      */
-    STEPS_EUNSUPPORTED = -5   /* a mode that this build does not contain (EWALD_TABLE)                 */
+    STEPS_EUNSUPPORTED = -5   /* a combination this build does not contain (EWALD_TABLE with mixed
+                                 precision or with STEPS_FLAG_DETERMINISTIC)                           */
 } steps_cyl_status;
 
 enum { STEPS_PERIODIC_IMAGES = 0,      /* Eq. 8, truncated image sum                                  */
-       STEPS_PERIODIC_EWALD_TABLE = 1  /* Eq. 12-17, lookup-table correction: not built yet            */ };
+       STEPS_PERIODIC_EWALD_TABLE = 1  /* Eq. 12-17: softened nearest image + interpolated table D;
+                                          fp64 precision only (mixed: STEPS_EUNSUPPORTED)              */ };
 enum { STEPS_PREC_FP64 = 0,            /* every pair term and the accumulation in double               */
        STEPS_PREC_MIXED = 1            /* pair terms in float (cancellation-safe separations),
                                           accumulation over sources in double                          */ };
+enum { STEPS_INTERP_CIC = 0,           /* cloud-in-cell: bilinear in (rho, z)                          */
+       STEPS_INTERP_TSC = 1            /* triangular-shaped cloud: quadratic B-spline on 3 x 3 nodes   */ };
 enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz                                    */
        STEPS_BG_INFINITE = 1           /* Eq. 10                                                       */ };
 
@@ -89,11 +93,21 @@ typedef struct {
     double  rho0;           /* comoving mean density of Eq. 9/10; 0 disables the background term      */
     int32_t device;         /* CUDA device ordinal                                                    */
     int32_t flags;          /* bitwise OR of STEPS_FLAG_*; 0 = defaults                               */
+    /* STEPS_PERIODIC_EWALD_TABLE only; zeros select the defaults in brackets   */
+    int32_t ew_nmax;        /* real-space images n = -nmax..nmax of Eq. 13        [5]                 */
+    int32_t ew_mmax;        /* Fourier modes m = 1..mmax of Eq. 14                [12]                */
+    double  ew_alpha;       /* Ewald split parameter alpha, 1/length              [2/Lz]              */
+    int32_t tab_nrho;       /* radial nodes of the table D(rho, z)                [144]               */
+    int32_t tab_nz;         /* axial nodes, z in [0, Lz/2]                        [128]               */
+    double  tab_rho_max;    /* radial extent of the table; beyond it the pair force is the line-mass
+                               term -2 G m/(Lz rho) e_rho (reading T2)            [5 Lz]              */
+    int32_t interp;         /* STEPS_INTERP_CIC or STEPS_INTERP_TSC                    */
+    int32_t reserved;       /* must be 0                                                              */
 } steps_cyl_params;
 
 /* Validate `p`, select the device, allocate scratch for n particles and build the constant
  * tables (image offsets, quadrature nodes of Eq. 9).  Host-synchronous.
- * Errors: EINVAL, EUNSUPPORTED (periodic_mode == EWALD_TABLE), ECUDA, ENOMEM. */
+ * Errors: EINVAL, EUNSUPPORTED, ECUDA, ENOMEM. */
 int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out);
 
 /* Free everything the context owns.  NULL is allowed. */
@@ -165,6 +179,15 @@ int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx,
  * with the N-body step dt.  Host only, no context.  EINVAL on NULL / a <= 0. */
 int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double Or, double Ok,
                              double OL, double *a_next, double *H_next);
+
+/* The correction lookup table of Eq. 17, D = F_{S1xR2} - F_{R3} per unit G m_i m_j (Ewald sum of
+ * Eq. 12-16 with the Fourier kernel of DESIGN.md reading G4, minus the unsoftened nearest-image
+ * force), on the grid rho_i = i rho_max/(nrho-1), z_j = j (Lz/2)/(nz-1).
+ * out: HOST pointer, nrho*nz*2 doubles, D[(i*nz + j)*2 + c], c = 0 radial, 1 axial.
+ * Host only, no context, no device.  EINVAL on NULL, Lz <= 0, alpha <= 0, nrho < 2, nz < 2,
+ * nmax < 0, mmax < 0, rho_max <= 0. */
+int steps_cyl_ewald_table(double Lz, double alpha, int32_t nmax, int32_t mmax, int32_t nrho,
+                          int32_t nz, double rho_max, double *out);
 
 /* Measured ceiling of the FP64 pipe: runs an unrolled chain of independent DFMAs on every SM
  * of the context's device for about `ms` milliseconds and returns DFMA instructions per

@@ -17,11 +17,12 @@ PERIODIC_IMAGES, PERIODIC_EWALD_TABLE = 0, 1
 PREC_FP64, PREC_MIXED = 0, 1
 BG_FINITE, BG_INFINITE = 0, 1
 FLAG_DETERMINISTIC = 1
+INTERP_CIC, INTERP_TSC = 0, 1
 
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",
            "steps_cyl_check", "steps_cyl_background", "steps_cyl_kdk_step",
            "steps_cyl_kdk_step_host",
-           "steps_cyl_friedmann_step", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
+           "steps_cyl_friedmann_step", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
            "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count"]
 
 
@@ -30,7 +31,10 @@ class Params(C.Structure):
     _fields_ = [("n", C.c_int64), ("Lz", C.c_double), ("G", C.c_double),
                 ("periodic_mode", C.c_int32), ("n_cut", C.c_int32), ("precision", C.c_int32),
                 ("background", C.c_int32), ("R_sim", C.c_double), ("rho0", C.c_double),
-                ("device", C.c_int32), ("flags", C.c_int32)]
+                ("device", C.c_int32), ("flags", C.c_int32),
+                ("ew_nmax", C.c_int32), ("ew_mmax", C.c_int32), ("ew_alpha", C.c_double),
+                ("tab_nrho", C.c_int32), ("tab_nz", C.c_int32), ("tab_rho_max", C.c_double),
+                ("interp", C.c_int32), ("reserved", C.c_int32)]
 
 
 class StepsError(RuntimeError):
@@ -69,6 +73,8 @@ def lib():
         L.steps_cyl_kdk_step_host.argtypes = [vp] + [dp] * 11 + [d] * 5
         L.steps_cyl_friedmann_step.restype = C.c_int
         L.steps_cyl_friedmann_step.argtypes = [d] * 7 + [C.POINTER(d), C.POINTER(d)]
+        L.steps_cyl_ewald_table.restype = C.c_int
+        L.steps_cyl_ewald_table.argtypes = [d, d, C.c_int32, C.c_int32, C.c_int32, C.c_int32, d, dp]
         L.steps_cyl_fp64_peak.restype = C.c_int
         L.steps_cyl_fp64_peak.argtypes = [vp, d, C.POINTER(d)]
         L.steps_cyl_last_pair_kernel_ms.restype = C.c_int
@@ -90,6 +96,17 @@ def friedmann_step(a, dt, H0, Om, Or=0.0, Ok=0.0, OL=0.0):
     if rc:
         raise StepsError(rc, lib().steps_cyl_strerror(rc).decode())
     return an.value, Hn.value
+
+
+def ewald_table(Lz, alpha, nmax, mmax, nrho, nz, rho_max):
+    """steps_cyl_ewald_table: the Eq. 17 correction table, D[nrho, nz, 2] (host only)."""
+    import numpy as np
+    D = np.zeros((int(nrho), int(nz), 2))
+    rc = lib().steps_cyl_ewald_table(float(Lz), float(alpha), int(nmax), int(mmax), int(nrho), int(nz),
+                                     float(rho_max), C.c_void_p(D.ctypes.data))
+    if rc:
+        raise StepsError(rc, lib().steps_cyl_strerror(rc).decode())
+    return D
 
 
 def _dev_ptr(t, n):
@@ -121,11 +138,16 @@ class StepsCyl:
     """One steps_cyl_ctx.  Methods mirror the C entry points one to one."""
 
     def __init__(self, n, Lz, G=1.0, n_cut=5, precision=PREC_FP64, background=BG_FINITE,
-                 R_sim=0.0, rho0=0.0, device=0, periodic_mode=PERIODIC_IMAGES, flags=0):
+                 R_sim=0.0, rho0=0.0, device=0, periodic_mode=PERIODIC_IMAGES, flags=0,
+                 ew_nmax=0, ew_mmax=0, ew_alpha=0.0, tab_nrho=0, tab_nz=0, tab_rho_max=0.0,
+                 interp=INTERP_CIC):
         self._ctx = C.c_void_p()
         self.params = Params(n=int(n), Lz=float(Lz), G=float(G), periodic_mode=int(periodic_mode),
                              n_cut=int(n_cut), precision=int(precision), background=int(background),
-                             R_sim=float(R_sim), rho0=float(rho0), device=int(device), flags=int(flags))
+                             R_sim=float(R_sim), rho0=float(rho0), device=int(device), flags=int(flags),
+                             ew_nmax=int(ew_nmax), ew_mmax=int(ew_mmax), ew_alpha=float(ew_alpha),
+                             tab_nrho=int(tab_nrho), tab_nz=int(tab_nz),
+                             tab_rho_max=float(tab_rho_max), interp=int(interp), reserved=0)
         self.n = int(n)
         rc = lib().steps_cyl_init(C.byref(self.params), C.byref(self._ctx))
         if rc:

@@ -16,6 +16,8 @@
 #include "pair_fp64_sym.cuh"
 #include "pair_mixed.cuh"
 #include "pair_mixed_sym.cuh"
+#include "pair_table_sym.cuh"
+#include "ewald_table.h"
 
 using namespace steps;
 
@@ -36,6 +38,9 @@ struct steps_cyl_ctx {
     double *bx = nullptr, *by = nullptr;          // background acceleration at the current x
     DevFlags *flags = nullptr;
     QuadNode *nodes = nullptr;
+    double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
+    TableConsts tc;
+    bool table_mode = false;
     int n_nodes = 0;
     double *host_io = nullptr;                     // device staging for the *_host entry points
     double *peak_out = nullptr;
@@ -147,6 +152,14 @@ void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 
 void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
+    if (c->table_mode) {
+        dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
+        pair_table_sym_kernel<<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad,
+                                                          c->n_tiles, c->sym_tiles_per_chunk, c->kc,
+                                                          c->tc, c->part);
+        c->launches += 1;
+        return;
+    }
     const bool mixed = c->p.precision == STEPS_PREC_MIXED;
     switch (c->p.n_cut) {
 #define CASE_NC(N)                                               \
@@ -190,7 +203,8 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
     ctx->ev_valid = true;
     finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
                                                          ctx->use_sym ? 1 : ctx->n_chunks,
-                                                         ctx->n_chunks, ctx->kc.halfL, ctx->flags,
+                                                         ctx->table_mode ? 1 : ctx->n_chunks,
+                                                         ctx->kc.halfL, ctx->flags,
                                                          ctx->p.G, ctx->p.Lz, gx, gy, gz);
     ctx->launches += 1;
     CK(cudaGetLastError());
@@ -220,18 +234,35 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     if (p->n < 1 || p->n >= (int64_t)2147483647 - 2 * PAIR_THREADS) return STEPS_EINVAL;
     if (!(p->Lz > 0.0) || !std::isfinite(p->Lz) || !std::isfinite(p->G)) return STEPS_EINVAL;
     if (p->n_cut < 1 || p->n_cut > 1000000) return STEPS_EINVAL;
-    if (p->periodic_mode == STEPS_PERIODIC_EWALD_TABLE) return STEPS_EUNSUPPORTED;
-    if (p->periodic_mode != STEPS_PERIODIC_IMAGES) return STEPS_EINVAL;
+    if (p->periodic_mode != STEPS_PERIODIC_IMAGES && p->periodic_mode != STEPS_PERIODIC_EWALD_TABLE)
+        return STEPS_EINVAL;
     if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
     if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
     if ((p->flags & ~STEPS_FLAG_DETERMINISTIC) != 0 || p->device < 0) return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
     if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
+    if (p->reserved != 0) return STEPS_EINVAL;
+    steps_cyl_params pp = *p;                      // table parameters with defaults filled in
+    if (p->periodic_mode == STEPS_PERIODIC_EWALD_TABLE) {
+        if (pp.ew_nmax == 0) pp.ew_nmax = 5;
+        if (pp.ew_mmax == 0) pp.ew_mmax = 12;
+        if (pp.ew_alpha == 0.0) pp.ew_alpha = 2.0 / p->Lz;
+        if (pp.tab_nrho == 0) pp.tab_nrho = 144;
+        if (pp.tab_nz == 0) pp.tab_nz = 128;
+        if (pp.tab_rho_max == 0.0) pp.tab_rho_max = 5.0 * p->Lz;
+        if (pp.ew_nmax < 0 || pp.ew_mmax < 0 || !(pp.ew_alpha > 0.0) || !std::isfinite(pp.ew_alpha) ||
+            pp.tab_nrho < 2 || pp.tab_nz < 2 || pp.tab_nrho > 16384 || pp.tab_nz > 16384 ||
+            !(pp.tab_rho_max > 0.0) || !std::isfinite(pp.tab_rho_max) ||
+            (pp.interp != STEPS_INTERP_CIC && pp.interp != STEPS_INTERP_TSC))
+            return STEPS_EINVAL;
+        if (p->precision != STEPS_PREC_FP64 || (p->flags & STEPS_FLAG_DETERMINISTIC))
+            return STEPS_EUNSUPPORTED;
+    }
 
     steps_cyl_ctx *ctx = new (std::nothrow) steps_cyl_ctx();
     if (!ctx) return STEPS_ENOMEM;
     ctx->cuda_msg[0] = 0;
-    ctx->p = *p;
+    ctx->p = pp;
     int rc = STEPS_OK;
     auto fail = [&](int code) { steps_cyl_destroy(ctx); return code; };
 
@@ -297,6 +328,24 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         if (rc == STEPS_OK) A(cudaMemcpy(ctx->nodes, v.data(), v.size() * sizeof(QuadNode), cudaMemcpyHostToDevice));
         if (rc != STEPS_OK) return fail(rc);
     }
+    if (pp.periodic_mode == STEPS_PERIODIC_EWALD_TABLE) {
+        ctx->table_mode = true;
+        const size_t nodes = (size_t)pp.tab_nrho * pp.tab_nz;
+        std::vector<double> D(nodes * 2);
+        build_ewald_table(pp.Lz, pp.ew_alpha, pp.ew_nmax, pp.ew_mmax, pp.tab_nrho, pp.tab_nz,
+                          pp.tab_rho_max, D.data());
+        A(dev_alloc(&ctx->d_table, nodes));
+        if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table, D.data(), nodes * sizeof(double2), cudaMemcpyHostToDevice));
+        if (rc != STEPS_OK) return fail(rc);
+        ctx->tc.D = ctx->d_table;
+        ctx->tc.nrho = pp.tab_nrho;
+        ctx->tc.nz = pp.tab_nz;
+        ctx->tc.interp = pp.interp;
+        ctx->tc.rho_max2 = pp.tab_rho_max * pp.tab_rho_max;
+        ctx->tc.inv_drho = (double)(pp.tab_nrho - 1) / pp.tab_rho_max;
+        ctx->tc.inv_dz = (double)(pp.tab_nz - 1) / (0.5 * pp.Lz);
+        ctx->tc.two_over_L = 2.0 / pp.Lz;
+    }
     A(cudaMemset(ctx->flags, 0, sizeof(DevFlags)));
     if (rc != STEPS_OK) return fail(rc);
     *out = ctx;
@@ -307,7 +356,7 @@ void steps_cyl_destroy(steps_cyl_ctx *c)
 {
     if (!c) return;
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes);
+    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -439,6 +488,16 @@ int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double O
     return STEPS_OK;
 }
 
+int steps_cyl_ewald_table(double Lz, double alpha, int32_t nmax, int32_t mmax, int32_t nrho,
+                          int32_t nz, double rho_max, double *out)
+{
+    if (!out || !(Lz > 0.0) || !(alpha > 0.0) || nrho < 2 || nz < 2 || nmax < 0 || mmax < 0 ||
+        !(rho_max > 0.0))
+        return STEPS_EINVAL;
+    build_ewald_table(Lz, alpha, nmax, mmax, nrho, nz, rho_max, out);
+    return STEPS_OK;
+}
+
 int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s)
 {
     if (!ctx || !dfma_per_s || !(ms > 0.0)) return STEPS_EINVAL;
@@ -486,7 +545,7 @@ const char *steps_cyl_strerror(int code)
     case STEPS_ESOFT: return "softening precondition violated (some h_i <= 0)";
     case STEPS_ECUDA: return "CUDA runtime error (see steps_cyl_last_cuda_error)";
     case STEPS_ENOMEM: return "out of memory";
-    case STEPS_EUNSUPPORTED: return "mode not built (EWALD_TABLE)";
+    case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE needs fp64 and no DETERMINISTIC flag)";
     default: return "unknown status";
     }
 }

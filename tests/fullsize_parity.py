@@ -31,9 +31,9 @@ def main():
     build.build()
     oracle.build()
     assert torch.cuda.is_available()
-    print("| config | N | mode | targets | max rel err | RMS rel err | median kappa | GPU s / evaluation | "
+    print("| config | N | mode | targets | max rel err | RMS rel err | GPU s / evaluation | "
           "sum m g / sum m abs(g) |")
-    print("|---|---:|---|---:|---:|---:|---:|---:|---:|")
+    print("|---|---:|---|---:|---:|---:|---:|---:|")
     for cfg in [int(c) for c in args.configs.split(",")]:
         w = workloads.make(cfg, n=args.n or None)
         idx = workloads.sample_targets(w.n, args.targets, seed=cfg)
@@ -56,7 +56,7 @@ def main():
             ctx.close()
             e = np.linalg.norm(got[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
             mom = max(abs(np.sum(w.m * got[:, c])) / np.sum(w.m * np.abs(got[:, c])) for c in range(3))
-            print("| %d | %d | %s | %d | %.2e | %.2e | | %.3f | %.1e |"
+            print("| %d | %d | %s | %d | %.2e | %.2e | %.3f | %.1e |"
                   % (cfg, w.n, name, len(idx), e.max(), np.sqrt(np.mean(e ** 2)), secs, mom), flush=True)
 
 

@@ -31,9 +31,15 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_params_struct_layout_matches_header():
     from paper_2602_20787_b200.binding import Params
-    # int64, double, double, 4 x int32, double, double, 2 x int32  -> 64 bytes, no padding surprises
-    assert C.sizeof(Params) == 64
+    # int64, 2 double, 4 int32, 2 double, 2 int32 | 2 int32, double, 2 int32, double, 2 int32
+    assert C.sizeof(Params) == 104
     assert Params.R_sim.offset == 40 and Params.device.offset == 56
+    assert Params.ew_alpha.offset == 72 and Params.tab_rho_max.offset == 88 and Params.interp.offset == 96
+    hdr = open(os.path.join(ROOT, "include", "steps_cyl.h")).read()
+    body = hdr[hdr.index("typedef struct {"):hdr.index("} steps_cyl_params;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = re.findall(r"\b(?:int64_t|int32_t|double)\s+(\w+)\s*;", body)
+    assert names == [f[0] for f in Params._fields_]
 
 
 def test_init_rejects_bad_arguments(lib):
@@ -47,8 +53,13 @@ def test_init_rejects_bad_arguments(lib):
         p = b.Params(**{**good, **bad})
         assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EINVAL, bad
         assert not ctx.value
-    p = b.Params(**{**good, "periodic_mode": b.PERIODIC_EWALD_TABLE})
-    assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EUNSUPPORTED
+    # EWALD_TABLE is fp64-only and has no ordered-pair kernel; bad table parameters are EINVAL
+    for extra in (dict(precision=b.PREC_MIXED), dict(flags=b.FLAG_DETERMINISTIC)):
+        p = b.Params(**{**good, "periodic_mode": b.PERIODIC_EWALD_TABLE, **extra})
+        assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EUNSUPPORTED
+    for extra in (dict(tab_nrho=1), dict(ew_alpha=-1.0), dict(interp=5), dict(tab_rho_max=-3.0), dict(reserved=1)):
+        p = b.Params(**{**good, "periodic_mode": b.PERIODIC_EWALD_TABLE, **extra})
+        assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EINVAL, extra
     assert lib.steps_cyl_init(None, C.byref(ctx)) == b.STEPS_EINVAL
     assert lib.steps_cyl_accel(None, *([None] * 8), None) == b.STEPS_EINVAL
     assert lib.steps_cyl_kdk_step(None, *([None] * 11), 1.0, 1.0, 1.0, 1.0, 1.0, None) == b.STEPS_EINVAL
@@ -101,3 +112,18 @@ def test_friedmann_step_lcdm_hubble_value(lib):
     assert H == pytest.approx(100.0 * math.sqrt(1e-4 / 0.5 ** 4 + 0.3 / 0.5 ** 3 + 0.7 - 1e-4), rel=1e-15)
     assert lib.steps_cyl_friedmann_step(-1.0, 0.1, 1.0, 1.0, 0.0, 0.0, 0.0, C.byref(C.c_double()),
                                         C.byref(C.c_double())) == b.STEPS_EINVAL
+
+
+def test_ewald_table_builder_matches_the_oracle_table(lib, oracle):
+    """steps_cyl_ewald_table (host-only entry point; double-exponential quadrature, own series) against
+    the oracle's table (Gauss-Legendre panels), written independently from Eq. 12-17."""
+    import numpy as np
+    from paper_2602_20787_b200 import binding as b
+    for (L, aL, nmax, mmax, nrho, nz, rmax) in [(100.0, 2.0, 5, 12, 19, 13, 450.0), (1.0, 3.0, 7, 14, 9, 9, 2.5)]:
+        got = b.ewald_table(L, aL / L, nmax, mmax, nrho, nz, rmax)
+        want = oracle.ewald_table(L, aL / L, nmax, mmax, nrho, nz, rmax)
+        scale = np.abs(want).max()
+        assert np.abs(got - want).max() <= 1e-12 * scale
+        nz_mask = np.abs(want) > 1e-6 * scale
+        assert np.abs(got[nz_mask] / want[nz_mask] - 1).max() <= 1e-9
+    assert lib.steps_cyl_ewald_table(1.0, 1.0, 5, 12, 1, 8, 1.0, None) == b.STEPS_EINVAL
