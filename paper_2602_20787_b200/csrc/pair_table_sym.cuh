@@ -26,6 +26,14 @@ struct TableConsts {
     double two_over_L;
 };
 
+// Exact nearest image, |r_z| <= L/2.  The high-word test of nearest_image() may leave |r_z| above
+// L/2 by a relative 2^-20 -- harmless for the symmetric image window of Eq. 8, but here the single
+// image that is kept, and the sign given to D_z, depend on it.
+__device__ __forceinline__ double nearest_image_exact(double rz, const PairConsts &k)
+{
+    return (fabs(rz) > k.halfL) ? rz - copysign(k.L, rz) : rz;
+}
+
 // 1/sqrt(x) to ~1 ulp for normal positive x (RSQ64H seed + one third-order step).
 __device__ __forceinline__ double rsqrt_full(double x)
 {
@@ -132,7 +140,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
-            const double rz = nearest_image(ti[r].z - pb.x, k);
+            const double rz = nearest_image_exact(ti[r].z - pb.x, k);
             double px, py, pz;
             table_pair(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, px, py, pz);
             a[r][0] = fma(pb.y, px, a[r][0]);
