@@ -41,6 +41,10 @@ KERNEL_MIX = {
     # STEPS_FLAG_DETERMINISTIC, pair_fp64_kernel<5,0>: one ordered pair per iteration
     "fp64_det": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
                      per_image=(9.5, 14.0)),
+    # --periodic table: pair_table_sym_kernel<CIC> (softened nearest image + 4 table gathers), one
+    # unordered pair per iteration; independent of n_cut
+    "table": dict(kernel="pair_table_sym_kernel<CIC>", interactions=2, dfma=22, dmul=14, dadd=14, dsetp=5,
+                  per_image=(0.0, 0.0)),
     # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
     # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
     "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=25, fmul=24, fadd=29, mufu=10,
@@ -65,7 +69,7 @@ def pipe_counts(mode, n_cut):
         return (instr + 7.5 * d) / mix["interactions"], (flops + 9.0 * d) / mix["interactions"]
     instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
     flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
-    d = 2 * (n_cut - 5)                                  # extra image terms per pair evaluation
+    d = 0 if mode == "table" else 2 * (n_cut - 5)        # extra image terms per pair evaluation
     instr += mix["per_image"][0] * d
     flops += mix["per_image"][1] * d
     return instr / mix["interactions"], flops / mix["interactions"]
@@ -219,8 +223,12 @@ def run_ours(args):
     # replicas only: every rank integrates its own particle set
     w = workloads.make(3, n=args.n, seed=3 + rank)
     n = w.n
-    ctx = b.StepsCyl(n=n, Lz=w.Lz, G=w.G, n_cut=args.n_cut, precision=prec, background=b.BG_FINITE,
+    table = args.periodic == "table"
+    # table mode sums all images (N_cut -> inf), so its consistent background term is Eq. 10
+    ctx = b.StepsCyl(n=n, Lz=w.Lz, G=w.G, n_cut=args.n_cut, precision=prec,
+                     background=b.BG_INFINITE if table else b.BG_FINITE,
                      R_sim=w.R_sim, rho0=w.rho0, device=local,
+                     periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
                      flags=b.FLAG_DETERMINISTIC if args.deterministic else 0)
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
@@ -283,7 +291,7 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peaks_kind = load_peaks()
-    mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
+    mode = "table" if table else ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
     instr, flops = pipe_counts(mode, args.n_cut)
     t_pair = float(np.mean(pair_ms)) * 1e-3
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
@@ -319,6 +327,8 @@ def run_ours(args):
         cpu = {"value": len(idx) * (n - 1) / tc, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
                          "%.1f s" % (len(idx), n, tc)}
+    periodic_desc = ("Ewald table 144x128 CIC, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10" if table
+                     else "n_cut=%d (%d images/pair), background Eq. 9" % (args.n_cut, 2 * args.n_cut))
     line = {
         "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
@@ -326,11 +336,10 @@ def run_ours(args):
         "dtype": "f64" if prec == b.PREC_FP64 else "f32",
         "data": "synthetic",
         "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving KDK step (Om=0.3, OL=0.7, "
-                               "a 0.02->0.025), L=100 Mpc/h, r_max=1000, n_cut=%d (10 images/pair), "
-                               "background Eq. 9" % (n, args.n_cut),
+                               "a 0.02->0.025), L=100 Mpc/h, r_max=1000, %s" % (n, periodic_desc),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between steps (L2 flush)"},
-        "image_terms_per_s": value * 2 * args.n_cut,
+        "image_terms_per_s": None if table else value * 2 * args.n_cut,
         "seconds_per_force_evaluation": t_pair,
         "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": 11 * 8 * n,
@@ -352,6 +361,8 @@ def main():
     ap.add_argument("--n", type=int, default=1048576)
     ap.add_argument("--n-cut", type=int, default=5)
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"])
+    ap.add_argument("--periodic", default="images", choices=["images", "table"],
+                    help="images: truncated image sum of Eq. 8 (the metric's mode); table: Eq. 12-17")
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per sample / reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -57,10 +57,11 @@ __device__ __forceinline__ double2 table_node(const TableConsts &tc, int i, int 
 }
 
 // Interpolated {D_rho, D_z} at (rho, az = |r_z|), rho < rho_max.
+template <int INTERP>
 __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rho, double az)
 {
     const double xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
-    if (tc.interp == 0) {
+    if (INTERP == 0) {
         int i0 = __double2int_rd(xr), j0 = __double2int_rd(xz);
         const double fr = xr - (double)i0, fz = xz - (double)j0;
         // a weight of exactly 0 multiplies the clamped node when rho or |r_z| sits on the last node
@@ -96,6 +97,7 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rh
 }
 
 // -f of one pair (see the header): (px, py, pz).
+template <int INTERP>
 __device__ __forceinline__ void table_pair(double rx, double ry, double rz, double hi, double hj,
                                            int soft_hi, const TableConsts &tc, double &px,
                                            double &py, double &pz)
@@ -110,7 +112,7 @@ __device__ __forceinline__ void table_pair(double rx, double ry, double rz, doub
             const double hh = hi + hj;
             if (q < hh * hh) w0 = spline_w(q, hh);
         }
-        const double2 Dv = table_lookup(tc, rho2 * y, fabs(rz));
+        const double2 Dv = table_lookup<INTERP>(tc, rho2 * y, fabs(rz));
         const double cr = fma(-Dv.x, y, w0);               // w0 - D_rho / rho
         px = cr * rx;
         py = cr * ry;
@@ -123,7 +125,7 @@ __device__ __forceinline__ void table_pair(double rx, double ry, double rz, doub
     }
 }
 
-template <int R, bool SYM>
+template <int INTERP, int R, bool SYM>
 __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const int (&soft_hi)[R],
                                                    const SymSrc *s_src, int lane,
                                                    const PairConsts &k, const TableConsts &tc,
@@ -142,7 +144,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
             const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
             const double rz = nearest_image_exact(ti[r].z - pb.x, k);
             double px, py, pz;
-            table_pair(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, px, py, pz);
+            table_pair<INTERP>(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, px, py, pz);
             a[r][0] = fma(pb.y, px, a[r][0]);
             a[r][1] = fma(pb.y, py, a[r][1]);
             a[r][2] = fma(pb.y, pz, a[r][2]);
@@ -163,6 +165,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
 
 // Same grid, decomposition and acc layout as pair_fp64_sym_kernel (A_z2 stays 0).  The spline
 // pre-test needs no restriction on max(h): only the nearest image is ever evaluated here.
+template <int INTERP>
 __global__ void __launch_bounds__(PAIR_THREADS, 4)
 pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                       const double *__restrict__ hs, const double *__restrict__ tile_hmax,
@@ -211,7 +214,7 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
             double bx = 0.0, by = 0.0, bz = 0.0;
             const SymSrc *sub = s_src + js * 32;
             if (t >= tb + SYM_R) {
-                ring_subtile_table<SYM_R, true>(ti, soft_hi, sub, lane, k, tc, a, bx, by, bz);
+                ring_subtile_table<INTERP, SYM_R, true>(ti, soft_hi, sub, lane, k, tc, a, bx, by, bz);
             } else {
 #pragma unroll
                 for (int r = 0; r < SYM_R; ++r) {
@@ -221,9 +224,9 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
                     double (&a1r)[1][3] = reinterpret_cast<double (&)[1][3]>(a[r]);
                     double cx = 0.0, cy = 0.0, cz = 0.0;
                     if (tb + r < t || js > w)
-                        ring_subtile_table<1, true>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
+                        ring_subtile_table<INTERP, 1, true>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
                     else if (js == w)
-                        ring_subtile_table<1, false>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
+                        ring_subtile_table<INTERP, 1, false>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
                     bx += cx; by += cy; bz += cz;
                 }
             }

@@ -154,9 +154,16 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
     if (c->table_mode) {
         dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
-        pair_table_sym_kernel<<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad,
-                                                          c->n_tiles, c->sym_tiles_per_chunk, c->kc,
-                                                          c->tc, c->part);
+        if (c->tc.interp == STEPS_INTERP_CIC)
+            pair_table_sym_kernel<0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+                                                                 c->n_pad, c->n_tiles,
+                                                                 c->sym_tiles_per_chunk, c->kc, c->tc,
+                                                                 c->part);
+        else
+            pair_table_sym_kernel<1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+                                                                 c->n_pad, c->n_tiles,
+                                                                 c->sym_tiles_per_chunk, c->kc, c->tc,
+                                                                 c->part);
         c->launches += 1;
         return;
     }
