@@ -124,6 +124,21 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(seconds, dist=None, device=None):
+    """Job time = the slowest rank's device time (all ranks call this; identity without a group)."""
+    if dist is None:
+        return float(seconds)
+    import torch
+    t = torch.tensor([float(seconds)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(pairs_per_rank_step, steps, world, seconds_max):
+    """Replicas only: whole-job pair interactions/s = all ranks' units / slowest rank."""
+    return world * pairs_per_rank_step * steps / seconds_max
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -264,12 +279,9 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else {}
     ctx.check()
-    ms = torch.tensor([ev[0].elapsed_time(ev[1])], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    t_dev = float(ms.item()) * 1e-3
+    t_dev = max_over_ranks(ev[0].elapsed_time(ev[1]) * 1e-3, dist, "cuda")
     pairs_per_step = float(n) * float(n - 1)
-    value = world * pairs_per_step * args.steps / t_dev
+    value = replica_throughput(pairs_per_step, args.steps, world, t_dev)
 
     # end to end: pinned host buffers through steps_cyl_kdk_step_host, copies inside the timing
     hs = [host[q] for q in names] + hg
@@ -280,10 +292,8 @@ def run_ours(args):
     for k in range(args.steps):
         ctx.kdk_step_host(*hs, *sched[args.warmup + args.steps + 1 + k], w.cosmo["dt"])
     torch.cuda.synchronize()
-    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * pairs_per_step * args.steps / float(te.item())
+    e2e_value = replica_throughput(pairs_per_step, args.steps, world,
+                                   max_over_ranks(time.perf_counter() - t0, dist, "cuda"))
     assert all(bool(torch.isfinite(t).all()) for t in hg)
 
     if rank != 0:
