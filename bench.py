@@ -244,6 +244,7 @@ def run_ours(args):
                      background=b.BG_INFINITE if table else b.BG_FINITE,
                      R_sim=w.R_sim, rho0=w.rho0, device=local,
                      periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
+                     tab_fp32=1 if (table and args.table_fp32) else 0,
                      flags=b.FLAG_DETERMINISTIC if args.deterministic else 0)
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
@@ -337,7 +338,8 @@ def run_ours(args):
         cpu = {"value": len(idx) * (n - 1) / tc, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
                          "%.1f s" % (len(idx), n, tc)}
-    periodic_desc = ("Ewald table 144x128 CIC, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10" if table
+    periodic_desc = ("Ewald table 144x128 CIC%s, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10"
+                     % (" (float nodes in shared memory)" if args.table_fp32 else "") if table
                      else "n_cut=%d (%d images/pair), background Eq. 9" % (args.n_cut, 2 * args.n_cut))
     line = {
         "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
@@ -375,6 +377,8 @@ def main():
                     help="images: truncated image sum of Eq. 8 (the metric's mode); table: Eq. 12-17")
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per sample / reference step")
+    ap.add_argument("--table-fp32", action="store_true",
+                    help="--periodic table: float table held in shared memory (tab_fp32 = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--deterministic", action="store_true",
                     help="fp64: ordered-pair kernel with fixed-order reduction (STEPS_FLAG_DETERMINISTIC)")

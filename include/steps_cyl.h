@@ -102,7 +102,10 @@ typedef struct {
     double  tab_rho_max;    /* radial extent of the table; beyond it the pair force is the line-mass
                                term -2 G m/(Lz rho) e_rho (reading T2)            [5 Lz]              */
     int32_t interp;         /* STEPS_INTERP_CIC or STEPS_INTERP_TSC                    */
-    int32_t reserved;       /* must be 0                                                              */
+    int32_t tab_fp32;       /* 0: table nodes in double, read from global memory;  1: nodes rounded to
+                               float and held in shared memory (the paper's (5,12) Ewald sum is itself
+                               single-precision accurate); needs nrho*nz*8 B + 56 KB of
+                               shared memory per SM (144 x 128 fits), else STEPS_EUNSUPPORTED          */
 } steps_cyl_params;
 
 /* Validate `p`, select the device, allocate scratch for n particles and build the constant

@@ -34,7 +34,7 @@ class Params(C.Structure):
                 ("device", C.c_int32), ("flags", C.c_int32),
                 ("ew_nmax", C.c_int32), ("ew_mmax", C.c_int32), ("ew_alpha", C.c_double),
                 ("tab_nrho", C.c_int32), ("tab_nz", C.c_int32), ("tab_rho_max", C.c_double),
-                ("interp", C.c_int32), ("reserved", C.c_int32)]
+                ("interp", C.c_int32), ("tab_fp32", C.c_int32)]
 
 
 class StepsError(RuntimeError):
@@ -140,14 +140,14 @@ class StepsCyl:
     def __init__(self, n, Lz, G=1.0, n_cut=5, precision=PREC_FP64, background=BG_FINITE,
                  R_sim=0.0, rho0=0.0, device=0, periodic_mode=PERIODIC_IMAGES, flags=0,
                  ew_nmax=0, ew_mmax=0, ew_alpha=0.0, tab_nrho=0, tab_nz=0, tab_rho_max=0.0,
-                 interp=INTERP_CIC):
+                 interp=INTERP_CIC, tab_fp32=0):
         self._ctx = C.c_void_p()
         self.params = Params(n=int(n), Lz=float(Lz), G=float(G), periodic_mode=int(periodic_mode),
                              n_cut=int(n_cut), precision=int(precision), background=int(background),
                              R_sim=float(R_sim), rho0=float(rho0), device=int(device), flags=int(flags),
                              ew_nmax=int(ew_nmax), ew_mmax=int(ew_mmax), ew_alpha=float(ew_alpha),
                              tab_nrho=int(tab_nrho), tab_nz=int(tab_nz),
-                             tab_rho_max=float(tab_rho_max), interp=int(interp), reserved=0)
+                             tab_rho_max=float(tab_rho_max), interp=int(interp), tab_fp32=int(tab_fp32))
         self.n = int(n)
         rc = lib().steps_cyl_init(C.byref(self.params), C.byref(self._ctx))
         if rc:

@@ -44,7 +44,22 @@ __device__ __forceinline__ double rsqrt_full(double x)
     return fma(y0 * e, p, y0);
 }
 
-__device__ __forceinline__ double2 table_node(const TableConsts &tc, int i, int j)
+// Where the nodes live: double2 in global memory (read through L1), or float2 in shared memory.
+struct GlobalTable {
+    const double2 *D;
+    __device__ __forceinline__ double2 node(int idx) const { return __ldg(D + idx); }
+};
+struct SharedTableF32 {
+    const float2 *D;
+    __device__ __forceinline__ double2 node(int idx) const
+    {
+        const float2 v = D[idx];
+        return make_double2((double)v.x, (double)v.y);
+    }
+};
+
+template <class Tab>
+__device__ __forceinline__ double2 table_node(const TableConsts &tc, const Tab &tab, int i, int j)
 {
     // boundary rules: D_rho odd in rho / even in z, D_z even in rho / odd in z, both periodic in z
     double sr = 1.0, sz = 1.0;
@@ -52,13 +67,14 @@ __device__ __forceinline__ double2 table_node(const TableConsts &tc, int i, int 
     if (i > tc.nrho - 1) i = tc.nrho - 1;
     if (j < 0) { j = -j; sz = -1.0; }
     if (j > tc.nz - 1) { j = 2 * (tc.nz - 1) - j; sz = -sz; }
-    const double2 v = __ldg(tc.D + (size_t)i * tc.nz + j);
+    const double2 v = tab.node(i * tc.nz + j);
     return make_double2(sr * v.x, sz * v.y);
 }
 
 // Interpolated {D_rho, D_z} at (rho, az = |r_z|), rho < rho_max.
-template <int INTERP>
-__device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rho, double az)
+template <int INTERP, class Tab>
+__device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Tab &tab, double rho,
+                                                double az)
 {
     const double xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
     if (INTERP == 0) {
@@ -68,10 +84,10 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rh
         const int i1 = min(i0 + 1, tc.nrho - 1), j1 = min(j0 + 1, tc.nz - 1);
         i0 = min(i0, tc.nrho - 1);
         j0 = min(j0, tc.nz - 1);
-        const double2 d00 = __ldg(tc.D + (size_t)i0 * tc.nz + j0);
-        const double2 d01 = __ldg(tc.D + (size_t)i0 * tc.nz + j1);
-        const double2 d10 = __ldg(tc.D + (size_t)i1 * tc.nz + j0);
-        const double2 d11 = __ldg(tc.D + (size_t)i1 * tc.nz + j1);
+        const double2 d00 = tab.node(i0 * tc.nz + j0);
+        const double2 d01 = tab.node(i0 * tc.nz + j1);
+        const double2 d10 = tab.node(i1 * tc.nz + j0);
+        const double2 d11 = tab.node(i1 * tc.nz + j1);
         const double ax = fma(fz, d01.x - d00.x, d00.x), bx = fma(fz, d11.x - d10.x, d10.x);
         const double ay = fma(fz, d01.y - d00.y, d00.y), by = fma(fz, d11.y - d10.y, d10.y);
         return make_double2(fma(fr, bx - ax, ax), fma(fr, by - ay, ay));
@@ -86,7 +102,7 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rh
         double rx = 0.0, ry = 0.0;
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const double2 v = table_node(tc, ic - 1 + a, jc - 1 + b);
+            const double2 v = table_node(tc, tab, ic - 1 + a, jc - 1 + b);
             rx = fma(wz[b], v.x, rx);
             ry = fma(wz[b], v.y, ry);
         }
@@ -97,10 +113,10 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, double rh
 }
 
 // -f of one pair (see the header): (px, py, pz).
-template <int INTERP>
+template <int INTERP, class Tab>
 __device__ __forceinline__ void table_pair(double rx, double ry, double rz, double hi, double hj,
-                                           int soft_hi, const TableConsts &tc, double &px,
-                                           double &py, double &pz)
+                                           int soft_hi, const TableConsts &tc, const Tab &tab,
+                                           double &px, double &py, double &pz)
 {
     const double rho2 = fma(ry, ry, rx * rx);
     // rho2 == 0: y = 0 kills the radial table term (D_rho(0) = 0 and no direction)
@@ -112,7 +128,7 @@ __device__ __forceinline__ void table_pair(double rx, double ry, double rz, doub
             const double hh = hi + hj;
             if (q < hh * hh) w0 = spline_w(q, hh);
         }
-        const double2 Dv = table_lookup<INTERP>(tc, rho2 * y, fabs(rz));
+        const double2 Dv = table_lookup<INTERP>(tc, tab, rho2 * y, fabs(rz));
         const double cr = fma(-Dv.x, y, w0);               // w0 - D_rho / rho
         px = cr * rx;
         py = cr * ry;
@@ -125,10 +141,11 @@ __device__ __forceinline__ void table_pair(double rx, double ry, double rz, doub
     }
 }
 
-template <int INTERP, int R, bool SYM>
+template <int INTERP, int R, bool SYM, class Tab>
 __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const int (&soft_hi)[R],
                                                    const SymSrc *s_src, int lane,
                                                    const PairConsts &k, const TableConsts &tc,
+                                                   const Tab &tab,
                                                    double (&a)[R][3], double &bx, double &by,
                                                    double &bz)
 {
@@ -144,7 +161,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
             const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
             const double rz = nearest_image_exact(ti[r].z - pb.x, k);
             double px, py, pz;
-            table_pair<INTERP>(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, px, py, pz);
+            table_pair<INTERP>(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, tab, px, py, pz);
             a[r][0] = fma(pb.y, px, a[r][0]);
             a[r][1] = fma(pb.y, py, a[r][1]);
             a[r][2] = fma(pb.y, pz, a[r][2]);
@@ -163,37 +180,55 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
     }
 }
 
-// Same grid, decomposition and acc layout as pair_fp64_sym_kernel (A_z2 stays 0).  The spline
-// pre-test needs no restriction on max(h): only the nearest image is ever evaluated here.
-template <int INTERP>
-__global__ void __launch_bounds__(PAIR_THREADS, 4)
+// Same decomposition and acc layout as pair_fp64_sym_kernel (A_z2 stays 0), generalised to TW warps:
+// a CTA owns (TW/4) * SYM_R target tiles -- warp w holds sub-block w % 4 of target tiles
+// tb + (w/4) * SYM_R + r -- and streams 128-source tiles.  grid = (n_tiles / tiles_per_cta, chunks).
+//   SMEM_TABLE = false: TW = 4, the table is read from global memory (double2 nodes);
+//   SMEM_TABLE = true : TW = 16 (one CTA per SM), the float2 table is copied to shared memory first,
+//                       dynamic shared memory = TW*3*128*8 bytes of accumulators + nodes * 8 bytes.
+// The spline pre-test needs no restriction on max(h): only the nearest image is evaluated here.
+template <int INTERP, int TW, bool SMEM_TABLE>
+__global__ void __launch_bounds__(TW * 32, SMEM_TABLE ? 1 : 4)
 pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                       const double *__restrict__ hs, const double *__restrict__ tile_hmax,
                       int n_pad, int n_tiles, int tiles_per_chunk, PairConsts k, TableConsts tc,
-                      double *__restrict__ acc)
+                      const float2 *__restrict__ table_f32, double *__restrict__ acc)
 {
-    const int tb = blockIdx.x * SYM_R;
+    constexpr int TILES_PER_CTA = (TW / 4) * SYM_R;
+    const int tb = blockIdx.x * TILES_PER_CTA;
     const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
     __shared__ SymSrc s_src[PAIR_THREADS];
-    __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    // dynamic shared memory: per-warp source accumulators s_b[TW][3][128], then the float2 table
+    extern __shared__ double s_dyn[];
+    double (*s_b)[3][PAIR_THREADS] = reinterpret_cast<double (*)[3][PAIR_THREADS]>(s_dyn);
+    float2 *s_table = reinterpret_cast<float2 *>(s_dyn + TW * 3 * PAIR_THREADS);
+
+    if (SMEM_TABLE) {
+        const int nodes = tc.nrho * tc.nz;
+        for (int q = threadIdx.x; q < nodes; q += TW * 32) s_table[q] = table_f32[q];
+    }
+    GlobalTable gtab{tc.D};
+    SharedTableF32 stab{s_table};
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int wq = w & 3;                                   // sub-block of the target tiles
+    const int tgt0 = tb + (w >> 2) * SYM_R;                 // this warp's first target tile
     SymTgt ti[SYM_R];
     double a[SYM_R][3];
 #pragma unroll
     for (int r = 0; r < SYM_R; ++r) {
-        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+        const int i = (tgt0 + r) * PAIR_THREADS + wq * 32 + lane;
         const double2 pi = xy[i], qi = zm[i];
         ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
         ti[r].mL = 0.0;
         a[r][0] = a[r][1] = a[r][2] = 0.0;
     }
     for (int t = t0; t < t1; ++t) {
-        const int j = t * PAIR_THREADS + threadIdx.x;
-        __syncthreads();
-        {
+        __syncthreads();                                    // previous flush done (and the table is in)
+        if (threadIdx.x < PAIR_THREADS) {
+            const int j = t * PAIR_THREADS + threadIdx.x;
             const double2 pj = xy[j], qj = zm[j];
             SymSrc v;
             v.x = pj.x; v.y = pj.y; v.z = qj.x; v.m = qj.y; v.h = hs[j]; v.pad = 0.0;
@@ -213,20 +248,32 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
         for (int js = 0; js < PAIR_THREADS / 32; ++js) {
             double bx = 0.0, by = 0.0, bz = 0.0;
             const SymSrc *sub = s_src + js * 32;
-            if (t >= tb + SYM_R) {
-                ring_subtile_table<INTERP, SYM_R, true>(ti, soft_hi, sub, lane, k, tc, a, bx, by, bz);
+            if (t >= tgt0 + SYM_R) {
+                if (SMEM_TABLE)
+                    ring_subtile_table<INTERP, SYM_R, true>(ti, soft_hi, sub, lane, k, tc, stab, a, bx, by, bz);
+                else
+                    ring_subtile_table<INTERP, SYM_R, true>(ti, soft_hi, sub, lane, k, tc, gtab, a, bx, by, bz);
             } else {
+                // a tile at or below this warp's own target tiles: target tile tgt0 + r meets source tile t
+                // only if t >= tgt0 + r; in its own tile the warp takes sub-tiles above its own both ways,
+                // its own target-side only, and leaves the ones below to their owners
 #pragma unroll
                 for (int r = 0; r < SYM_R; ++r) {
-                    if (tb + r > t) continue;
+                    if (tgt0 + r > t) continue;
                     const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
                     const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
                     double (&a1r)[1][3] = reinterpret_cast<double (&)[1][3]>(a[r]);
                     double cx = 0.0, cy = 0.0, cz = 0.0;
-                    if (tb + r < t || js > w)
-                        ring_subtile_table<INTERP, 1, true>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
-                    else if (js == w)
-                        ring_subtile_table<INTERP, 1, false>(t1r, s1r, sub, lane, k, tc, a1r, cx, cy, cz);
+                    const bool both = (tgt0 + r < t) || (js > wq);
+                    if (both || js == wq) {
+                        if (SMEM_TABLE) {
+                            if (both) ring_subtile_table<INTERP, 1, true>(t1r, s1r, sub, lane, k, tc, stab, a1r, cx, cy, cz);
+                            else      ring_subtile_table<INTERP, 1, false>(t1r, s1r, sub, lane, k, tc, stab, a1r, cx, cy, cz);
+                        } else {
+                            if (both) ring_subtile_table<INTERP, 1, true>(t1r, s1r, sub, lane, k, tc, gtab, a1r, cx, cy, cz);
+                            else      ring_subtile_table<INTERP, 1, false>(t1r, s1r, sub, lane, k, tc, gtab, a1r, cx, cy, cz);
+                        }
+                    }
                     bx += cx; by += cy; bz += cz;
                 }
             }
@@ -236,17 +283,17 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
             s_b[w][2][jl] = bz;
         }
         __syncthreads();
+        for (int q = threadIdx.x; q < 3 * PAIR_THREADS; q += TW * 32) {
+            const int c = q / PAIR_THREADS, jl = q % PAIR_THREADS;
+            double v = s_b[0][c][jl];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            double v = s_b[0][c][threadIdx.x];
-#pragma unroll
-            for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
-            if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
+            for (int ww = 1; ww < TW; ++ww) v += s_b[ww][c][jl];
+            if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + t * PAIR_THREADS + jl, -v);
         }
     }
 #pragma unroll
     for (int r = 0; r < SYM_R; ++r) {
-        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+        const int i = (tgt0 + r) * PAIR_THREADS + wq * 32 + lane;
 #pragma unroll
         for (int c = 0; c < 3; ++c) atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
     }

@@ -39,6 +39,8 @@ struct steps_cyl_ctx {
     DevFlags *flags = nullptr;
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
+    float2 *d_table_f32 = nullptr;                 // the same rounded to float (tab_fp32), staged in smem
+    size_t table_smem_bytes = 0;
     TableConsts tc;
     bool table_mode = false;
     int n_nodes = 0;
@@ -154,16 +156,26 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
     if (c->table_mode) {
         dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
-        if (c->tc.interp == STEPS_INTERP_CIC)
-            pair_table_sym_kernel<0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
-                                                                 c->n_pad, c->n_tiles,
-                                                                 c->sym_tiles_per_chunk, c->kc, c->tc,
-                                                                 c->part);
-        else
-            pair_table_sym_kernel<1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
-                                                                 c->n_pad, c->n_tiles,
-                                                                 c->sym_tiles_per_chunk, c->kc, c->tc,
-                                                                 c->part);
+        const size_t sb4 = 4 * 3 * PAIR_THREADS * sizeof(double);
+        if (c->d_table_f32) {
+            dim3 g16(c->n_tiles / (4 * SYM_R), c->sym_chunks);
+            if (c->tc.interp == STEPS_INTERP_CIC)
+                pair_table_sym_kernel<0, 16, true><<<g16, 512, c->table_smem_bytes, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->kc,
+                    c->tc, c->d_table_f32, c->part);
+            else
+                pair_table_sym_kernel<1, 16, true><<<g16, 512, c->table_smem_bytes, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->kc,
+                    c->tc, c->d_table_f32, c->part);
+        } else if (c->tc.interp == STEPS_INTERP_CIC) {
+            pair_table_sym_kernel<0, 4, false><<<grid, PAIR_THREADS, sb4, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->kc, c->tc,
+                nullptr, c->part);
+        } else {
+            pair_table_sym_kernel<1, 4, false><<<grid, PAIR_THREADS, sb4, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->kc, c->tc,
+                nullptr, c->part);
+        }
         c->launches += 1;
         return;
     }
@@ -248,7 +260,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     if ((p->flags & ~STEPS_FLAG_DETERMINISTIC) != 0 || p->device < 0) return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
     if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
-    if (p->reserved != 0) return STEPS_EINVAL;
+    if (p->tab_fp32 != 0 && p->tab_fp32 != 1) return STEPS_EINVAL;
     steps_cyl_params pp = *p;                      // table parameters with defaults filled in
     if (p->periodic_mode == STEPS_PERIODIC_EWALD_TABLE) {
         if (pp.ew_nmax == 0) pp.ew_nmax = 5;
@@ -282,7 +294,10 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
 
     ctx->n = (int)p->n;
     // a multiple of SYM_R tiles: the symmetric kernel's CTAs own SYM_R target tiles each
-    ctx->n_tiles = SYM_R * ((ctx->n + SYM_R * PAIR_THREADS - 1) / (SYM_R * PAIR_THREADS));
+    {
+        const int tile_group = (pp.periodic_mode == STEPS_PERIODIC_EWALD_TABLE && pp.tab_fp32) ? 4 * SYM_R : SYM_R;
+        ctx->n_tiles = tile_group * ((ctx->n + tile_group * PAIR_THREADS - 1) / (tile_group * PAIR_THREADS));
+    }
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
     ctx->use_sym = !(p->flags & STEPS_FLAG_DETERMINISTIC);
@@ -344,6 +359,19 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         A(dev_alloc(&ctx->d_table, nodes));
         if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table, D.data(), nodes * sizeof(double2), cudaMemcpyHostToDevice));
         if (rc != STEPS_OK) return fail(rc);
+        if (pp.tab_fp32) {
+            // table rounded to float and staged in shared memory by a 512-thread CTA per SM
+            ctx->table_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(double) + nodes * sizeof(float2);
+            if (ctx->table_smem_bytes + sizeof(SymSrc) * PAIR_THREADS > (size_t)prop.sharedMemPerBlockOptin)
+                return fail(STEPS_EUNSUPPORTED);
+            std::vector<float> Df(nodes * 2);
+            for (size_t q = 0; q < nodes * 2; ++q) Df[q] = (float)D[q];
+            A(dev_alloc(&ctx->d_table_f32, nodes));
+            if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table_f32, Df.data(), nodes * sizeof(float2), cudaMemcpyHostToDevice));
+            A(cudaFuncSetAttribute(pair_table_sym_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_sym_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
+            if (rc != STEPS_OK) return fail(rc);
+        }
         ctx->tc.D = ctx->d_table;
         ctx->tc.nrho = pp.tab_nrho;
         ctx->tc.nz = pp.tab_nz;
@@ -363,7 +391,7 @@ void steps_cyl_destroy(steps_cyl_ctx *c)
 {
     if (!c) return;
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table);
+    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);

@@ -99,3 +99,24 @@ def test_table_mode_tracks_the_many_image_sum(torch_cuda):
                           tab_rho_max=120.0)
     e40, e5 = rel_err(tab, images(40)), rel_err(images(5), images(40))
     assert np.median(e40) < 0.2 * np.median(e5)
+
+
+@pytest.mark.parametrize("interp", [0, 1])
+def test_table_mode_fp32_table_in_shared_memory(torch_cuda, oracle, interp):
+    """tab_fp32 = 1: the nodes are rounded to float and held in shared memory (512-thread CTAs, eight
+    target tiles each).  The oracle gets ITS table rounded the same way; all arithmetic stays double.
+    Ragged N (not a multiple of 1024) and pairs beyond rho_max included."""
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(1, n=7001, seed=31)
+    nrho, nz, rmax = 144, 128, 5.0 * w.Lz
+    D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, nrho, nz, rmax)
+    D32 = D.astype(np.float32).astype(np.float64)
+    ref = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D32, rmax, interp)
+    g = gpu_accel_table(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, interp=interp, tab_fp32=1)
+    # a node whose double value sits within 1e-12 of a float rounding boundary may round differently on
+    # the two sides (one float ulp, 6e-8 of that node); diluted over the ~18000 nodes a particle's pairs
+    # touch this stays far below the bar
+    assert rel_err(g, ref).max() <= 1e-10
+    # and the float table changes the answer itself only at the 1e-8 level
+    ref64 = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, interp)
+    assert rel_err(g, ref64).max() <= 1e-6
