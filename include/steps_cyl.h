@@ -183,6 +183,13 @@ int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx,
 int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double Or, double Ok,
                              double OL, double *a_next, double *H_next);
 
+/* The same step for a Chevallier-Polarski-Linder dark energy, Eq. 18-20:
+ * O_DE(a) = ODE exp[-3 int_1^a (1 + w(a'))/a' da'], w(a) = w0 + wa (1 - a), i.e.
+ * O_DE(a) = ODE a^(-3 (1 + w0 + wa)) exp(3 wa (a - 1)).  w0 = -1, wa = 0 is steps_cyl_friedmann_step with
+ * OL = ODE; wa = 0 is wCDM.  Host only, no context.  EINVAL on NULL / a <= 0. */
+int steps_cyl_friedmann_step_cpl(double a, double dt, double H0, double Om, double Or, double Ok,
+                                 double ODE, double w0, double wa, double *a_next, double *H_next);
+
 /* The correction lookup table of Eq. 17, D = F_{S1xR2} - F_{R3} per unit G m_i m_j (Ewald sum of
  * Eq. 12-16 with the Fourier kernel of DESIGN.md reading G4, minus the unsoftened nearest-image
  * force), on the grid rho_i = i rho_max/(nrho-1), z_j = j (Lz/2)/(nz-1).

@@ -67,6 +67,12 @@ def lib():
         _lib.oracle_friedmann_rk4.argtypes = [d] * 7 + [p, p]
         _lib.oracle_background.restype = None
         _lib.oracle_background.argtypes = [i64, p, p, d, d, d, d, i, p, p]
+        _lib.oracle_omega_de.restype = d
+        _lib.oracle_omega_de.argtypes = [d] * 4
+        _lib.oracle_hubble_cpl.restype = d
+        _lib.oracle_hubble_cpl.argtypes = [d] * 8
+        _lib.oracle_friedmann_rk4_cpl.restype = None
+        _lib.oracle_friedmann_rk4_cpl.argtypes = [d] * 9 + [p, p]
         _lib.oracle_ewald_force.restype = None
         _lib.oracle_ewald_force.argtypes = [d, d, d, d, i, i, p]
         _lib.oracle_ewald_D.restype = None
@@ -214,3 +220,18 @@ def accel_table(x, y, z, m, h, L, G, D, rho_max, interp, targets=None, nthreads=
     if rc:
         raise ValueError("oracle_accel_table: bad arguments")
     return gx, gy, gz
+
+
+def omega_de(a, ODE, w0, wa):
+    """Eq. 19 with the CPL equation of state Eq. 20 (integral done numerically)."""
+    return lib().oracle_omega_de(float(a), float(ODE), float(w0), float(wa))
+
+
+def hubble_cpl(a, H0, Om, Or, Ok, ODE, w0, wa):
+    return lib().oracle_hubble_cpl(*map(float, (a, H0, Om, Or, Ok, ODE, w0, wa)))
+
+
+def friedmann_rk4_cpl(a, dt, H0, Om, Or, Ok, ODE, w0, wa):
+    an, Hn = C.c_double(), C.c_double()
+    lib().oracle_friedmann_rk4_cpl(*map(float, (a, dt, H0, Om, Or, Ok, ODE, w0, wa)), C.byref(an), C.byref(Hn))
+    return an.value, Hn.value

@@ -554,3 +554,47 @@ int oracle_accel_table(int64_t n, const double *x, const double *y, const double
     free(zw);
     return 0;
 }
+
+/* ------------------------------------------------------------- Eq. 18-20
+ * Friedmann equation with CPL dark energy, PAPER.md:168-183:
+ *   H^2 = H0^2 [ Or a^-4 + Om a^-3 + Ok a^-2 + O_DE(a) ],
+ *   O_DE(a) = O_DE0 exp[ -3 int_1^a (1 + w(a'))/a' da' ]   (Eq. 19),   w(a) = w0 + wa (1 - a)   (Eq. 20).
+ * The integral of Eq. 19 is done numerically as printed (composite 20-point Gauss-Legendre in
+ * ln a'); tests pin it to the closed form and to the constant-w power law. */
+double oracle_omega_de(double a, double ODE, double w0, double wa)
+{
+    double u1 = log(a);                       /* int_1^a (1+w)/a' da' = int_0^{ln a} (1 + w(e^u)) du */
+    int np = 8;
+    double hp = u1 / np, sum = 0.0;
+    for (int i = 0; i < np; ++i) {
+        double c = (i + 0.5) * hp, hw = 0.5 * hp;
+        for (int q = 0; q < 10; ++q)
+            for (int sg = -1; sg <= 1; sg += 2) {
+                double u = c + sg * hw * GL20_X[q];
+                sum += hw * GL20_W[q] * (1.0 + w0 + wa * (1.0 - exp(u)));
+            }
+    }
+    return ODE * exp(-3.0 * sum);
+}
+
+double oracle_hubble_cpl(double a, double H0, double Om, double Or, double Ok, double ODE,
+                         double w0, double wa)
+{
+    return H0 * sqrt(Or / (a * a * a * a) + Om / (a * a * a) + Ok / (a * a)
+                     + oracle_omega_de(a, ODE, w0, wa));
+}
+
+void oracle_friedmann_rk4_cpl(double a, double dt, double H0, double Om, double Or, double Ok,
+                              double ODE, double w0, double wa, double *a_next, double *H_next)
+{
+    double k1 = a * oracle_hubble_cpl(a, H0, Om, Or, Ok, ODE, w0, wa);
+    double a2 = a + 0.5 * dt * k1;
+    double k2 = a2 * oracle_hubble_cpl(a2, H0, Om, Or, Ok, ODE, w0, wa);
+    double a3 = a + 0.5 * dt * k2;
+    double k3 = a3 * oracle_hubble_cpl(a3, H0, Om, Or, Ok, ODE, w0, wa);
+    double a4 = a + dt * k3;
+    double k4 = a4 * oracle_hubble_cpl(a4, H0, Om, Or, Ok, ODE, w0, wa);
+    double an = a + dt * (k1 + 2.0 * k2 + 2.0 * k3 + k4) / 6.0;
+    *a_next = an;
+    *H_next = oracle_hubble_cpl(an, H0, Om, Or, Ok, ODE, w0, wa);
+}

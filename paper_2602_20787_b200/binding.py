@@ -22,7 +22,7 @@ INTERP_CIC, INTERP_TSC = 0, 1
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",
            "steps_cyl_check", "steps_cyl_background", "steps_cyl_kdk_step",
            "steps_cyl_kdk_step_host",
-           "steps_cyl_friedmann_step", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
+           "steps_cyl_friedmann_step", "steps_cyl_friedmann_step_cpl", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
            "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count"]
 
 
@@ -73,6 +73,8 @@ def lib():
         L.steps_cyl_kdk_step_host.argtypes = [vp] + [dp] * 11 + [d] * 5
         L.steps_cyl_friedmann_step.restype = C.c_int
         L.steps_cyl_friedmann_step.argtypes = [d] * 7 + [C.POINTER(d), C.POINTER(d)]
+        L.steps_cyl_friedmann_step_cpl.restype = C.c_int
+        L.steps_cyl_friedmann_step_cpl.argtypes = [d] * 9 + [C.POINTER(d), C.POINTER(d)]
         L.steps_cyl_ewald_table.restype = C.c_int
         L.steps_cyl_ewald_table.argtypes = [d, d, C.c_int32, C.c_int32, C.c_int32, C.c_int32, d, dp]
         L.steps_cyl_fp64_peak.restype = C.c_int
@@ -93,6 +95,15 @@ def friedmann_step(a, dt, H0, Om, Or=0.0, Ok=0.0, OL=0.0):
     """steps_cyl_friedmann_step: one RK4 step of Eq. 18; returns (a_next, H_next).  Host only."""
     an, Hn = C.c_double(), C.c_double()
     rc = lib().steps_cyl_friedmann_step(a, dt, H0, Om, Or, Ok, OL, C.byref(an), C.byref(Hn))
+    if rc:
+        raise StepsError(rc, lib().steps_cyl_strerror(rc).decode())
+    return an.value, Hn.value
+
+
+def friedmann_step_cpl(a, dt, H0, Om, Or, Ok, ODE, w0, wa):
+    """steps_cyl_friedmann_step_cpl: RK4 step of Eq. 18 with CPL dark energy (Eq. 19-20)."""
+    an, Hn = C.c_double(), C.c_double()
+    rc = lib().steps_cyl_friedmann_step_cpl(a, dt, H0, Om, Or, Ok, ODE, w0, wa, C.byref(an), C.byref(Hn))
     if rc:
         raise StepsError(rc, lib().steps_cyl_strerror(rc).decode())
     return an.value, Hn.value

@@ -523,6 +523,30 @@ int steps_cyl_friedmann_step(double a, double dt, double H0, double Om, double O
     return STEPS_OK;
 }
 
+// Eq. 19-20 in closed form: int_1^a (1 + w0 + wa (1 - a'))/a' da' = (1 + w0 + wa) ln a - wa (a - 1).
+static double hubble_cpl_of_a(double a, double H0, double Om, double Or, double Ok, double ODE,
+                              double w0, double wa)
+{
+    const double ia = 1.0 / a;
+    const double de = ODE * std::pow(a, -3.0 * (1.0 + w0 + wa)) * std::exp(3.0 * wa * (a - 1.0));
+    return H0 * std::sqrt(((Or * ia + Om) * ia + Ok) * ia * ia + de);
+}
+
+int steps_cyl_friedmann_step_cpl(double a, double dt, double H0, double Om, double Or, double Ok,
+                                 double ODE, double w0, double wa, double *a_next, double *H_next)
+{
+    if (!a_next || !H_next || !(a > 0.0)) return STEPS_EINVAL;
+    auto f = [&](double s) { return s * hubble_cpl_of_a(s, H0, Om, Or, Ok, ODE, w0, wa); };
+    const double k1 = f(a);
+    const double k2 = f(a + 0.5 * dt * k1);
+    const double k3 = f(a + 0.5 * dt * k2);
+    const double k4 = f(a + dt * k3);
+    const double an = a + dt / 6.0 * (k1 + 2.0 * (k2 + k3) + k4);
+    *a_next = an;
+    *H_next = hubble_cpl_of_a(an, H0, Om, Or, Ok, ODE, w0, wa);
+    return STEPS_OK;
+}
+
 int steps_cyl_ewald_table(double Lz, double alpha, int32_t nmax, int32_t mmax, int32_t nrho,
                           int32_t nz, double rho_max, double *out)
 {

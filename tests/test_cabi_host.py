@@ -127,3 +127,16 @@ def test_ewald_table_builder_matches_the_oracle_table(lib, oracle):
         nz_mask = np.abs(want) > 1e-6 * scale
         assert np.abs(got[nz_mask] / want[nz_mask] - 1).max() <= 1e-9
     assert lib.steps_cyl_ewald_table(1.0, 1.0, 5, 12, 1, 8, 1.0, None) == b.STEPS_EINVAL
+
+
+def test_friedmann_step_cpl_matches_oracle_and_lcdm(lib, oracle):
+    from paper_2602_20787_b200 import binding as b
+    for w0, wa in [(-1.0, 0.0), (-0.9, 0.0), (-0.95, 0.3), (-1.1, -0.5)]:
+        a, o = 0.02, 0.02
+        for _ in range(20):
+            a, H = b.friedmann_step_cpl(a, 2e-6, 100.0, 0.3, 8e-5, 0.0, 0.7, w0, wa)
+            o, Ho = oracle.friedmann_rk4_cpl(o, 2e-6, 100.0, 0.3, 8e-5, 0.0, 0.7, w0, wa)
+        assert a == pytest.approx(o, rel=1e-13) and H == pytest.approx(Ho, rel=1e-13)
+    a1, H1 = b.friedmann_step(0.5, 1e-3, 70.0, 0.3, 0.0, 0.0, 0.7)
+    a2, H2 = b.friedmann_step_cpl(0.5, 1e-3, 70.0, 0.3, 0.0, 0.0, 0.7, -1.0, 0.0)
+    assert a2 == pytest.approx(a1, rel=1e-15) and H2 == pytest.approx(H1, rel=1e-15)

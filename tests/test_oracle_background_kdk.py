@@ -203,3 +203,34 @@ def test_kdk_background_cancels_homogeneous_drag_free_case(oracle):
     rho = np.hypot(x0, y0)
     np.testing.assert_allclose(np.hypot(bx, by), [-oracle.Fh(r, R, ncut * L, G, rho0) for r in rho], rtol=1e-13)
     assert np.all(bx * x0 + by * y0 > 0)
+
+
+# ------------------------------------------------------------- Eq. 19-20: CPL dark energy
+def test_cpl_dark_energy_density(oracle):
+    """Eq. 19 integrated numerically by the oracle against (i) the textbook constant-w power law
+    a^(-3(1+w)), (ii) the closed form of the CPL integral, (iii) 30-digit quadrature of Eq. 19."""
+    import mpmath as mp
+    assert oracle.omega_de(0.3, 0.7, -1.0, 0.0) == pytest.approx(0.7, rel=1e-14)          # Lambda
+    for w in (-0.8, -1.2, 0.0, 1.0 / 3.0):
+        assert oracle.omega_de(0.25, 0.7, w, 0.0) == pytest.approx(0.7 * 0.25 ** (-3 * (1 + w)), rel=1e-13)
+    for a, w0, wa in [(0.02, -0.9, 0.3), (0.5, -1.1, -0.4), (1.7, -0.7, 0.2)]:
+        closed = 0.7 * a ** (-3 * (1 + w0 + wa)) * math.exp(3 * wa * (a - 1))
+        quad = 0.7 * mp.exp(-3 * mp.quad(lambda x: (1 + w0 + wa * (1 - x)) / x, [1, a]))
+        assert oracle.omega_de(a, 0.7, w0, wa) == pytest.approx(closed, rel=1e-13)
+        assert oracle.omega_de(a, 0.7, w0, wa) == pytest.approx(float(quad), rel=1e-13)
+
+
+def test_cpl_friedmann_reduces_and_has_closed_form(oracle):
+    # w0 = -1, wa = 0: identical to the Lambda-CDM step
+    a1, H1 = oracle.friedmann_rk4(0.3, 1e-4, 70.0, 0.3, 1e-4, 0.0, 0.7)
+    a2, H2 = oracle.friedmann_rk4_cpl(0.3, 1e-4, 70.0, 0.3, 1e-4, 0.0, 0.7, -1.0, 0.0)
+    assert a2 == pytest.approx(a1, rel=1e-15) and H2 == pytest.approx(H1, rel=1e-14)
+    # dark energy with w = 0 dilutes like matter: Om + ODE = 1 is Einstein-de Sitter, a = (3 H0 t/2)^(2/3)
+    H0, n = 70.0, 200
+    a0, a_end = 0.1, 0.2
+    dt = (2 / (3 * H0)) * (a_end ** 1.5 - a0 ** 1.5) / n
+    a = a0
+    for _ in range(n):
+        a, H = oracle.friedmann_rk4_cpl(a, dt, H0, 0.3, 0.0, 0.0, 0.7, 0.0, 0.0)
+    assert a == pytest.approx(a_end, rel=1e-10)
+    assert H == pytest.approx(H0 * a ** -1.5, rel=1e-12)
