@@ -219,6 +219,73 @@ def clustered(n: int = 4194304, seed: int = 4, n_spheres: int = 512, scale: floa
     return w
 
 
+# ------------------------------------------- paper-faithful particle load (Sect. 3.1, Eq. 21-22)
+def stereographic_load(n_target: int = 200000, D_s: float = 70.0, R_sim: float = 500.0,
+                       omega_c: float = 1.63973, Lz: float = 500.0, rho_bar: float = 1.0,
+                       eps_core: float | None = None, seed: int = 5) -> Workload:
+    """Initial particle load of the cylindrical StePS geometry: the radial
+    coordinate is compactified by the inverse stereographic map omega = 2 arctan(rho/D_s) (Eq. 21), the
+    compact domain is tessellated uniformly in (omega, phi, z), one particle sits at a random place in
+    each cell and carries m_i = rho_bar V_i with V_i the cell's volume in the non-compact
+    (rho, phi, z) coordinates; inside the core omega < omega_c the mass resolution is constant
+    (equal-volume cells).  Positions come back through rho = D_s tan(omega/2) (Eq. 22).
+    Defaults are the parameters of the paper's Fig. 4 (rho_c = D_s tan(omega_c/2) = 75.0 Mpc) at a
+    reduced particle number.  Softening: eps_core m^(1/3) scaling as in the BASELINE configs."""
+    rng = np.random.default_rng(seed)
+    rho_c = D_s * math.tan(0.5 * omega_c)
+    omega_max = 2.0 * math.atan(R_sim / D_s)
+    # cell sizes: d_omega, d_phi, d_z chosen so that the first ring outside the core is roughly cubic
+    # and the total count is close to n_target
+    jac_c = 0.5 * D_s / math.cos(0.5 * omega_c) ** 2                 # d rho / d omega at omega_c
+    def counts(cell):                                              # cell = physical edge at rho_c
+        n_z = max(1, round(Lz / cell))
+        n_phi = max(4, round(2.0 * math.pi * rho_c / cell))
+        n_om = max(1, round((omega_max - omega_c) / (cell / jac_c)))
+        v_first = 0.5 * ((D_s * math.tan(0.5 * (omega_c + (omega_max - omega_c) / n_om))) ** 2 - rho_c ** 2) \
+            * (2.0 * math.pi / n_phi) * (Lz / n_z)
+        n_r = max(1, round(math.pi * rho_c ** 2 * Lz / v_first / (n_phi * n_z)))
+        return n_z, n_phi, n_om, n_r
+    lo, hi = 1e-3 * rho_c, 10.0 * rho_c
+    for _ in range(60):                                            # bisection on the cell edge
+        mid = math.sqrt(lo * hi)
+        n_z, n_phi, n_om, n_r = counts(mid)
+        if n_z * n_phi * (n_om + n_r) > n_target:
+            lo = mid
+        else:
+            hi = mid
+    n_z, n_phi, n_om, n_r = counts(hi)
+    d_phi, d_z = 2.0 * math.pi / n_phi, Lz / n_z
+    # outer region: uniform rings in omega
+    om_edges = np.linspace(omega_c, omega_max, n_om + 1)
+    rho_edges_out = D_s * np.tan(0.5 * om_edges)
+    # core: rings of equal area (constant mass resolution)
+    rho_edges_in = rho_c * np.sqrt(np.linspace(0.0, 1.0, n_r + 1))
+    xs, ys, zs, ms = [], [], [], []
+    for compact, edges in ((False, rho_edges_in), (True, rho_edges_out)):
+        nr = len(edges) - 1
+        shape = (nr, n_phi, n_z)
+        u = rng.random(shape)
+        if compact:      # random place in the COMPACT cell: uniform in omega
+            om = om_edges[:-1, None, None] + u * np.diff(om_edges)[:, None, None]
+            rho = D_s * np.tan(0.5 * om)
+        else:            # equal-volume core cell: uniform in rho^2
+            rho = np.sqrt(edges[:-1, None, None] ** 2 + u * np.diff(edges ** 2)[:, None, None])
+        phi = (np.arange(n_phi)[None, :, None] + rng.random(shape)) * d_phi
+        z = (np.arange(n_z)[None, None, :] + rng.random(shape)) * d_z
+        vol = 0.5 * np.diff(edges ** 2)[:, None, None] * d_phi * d_z * np.ones(shape)
+        xs.append((rho * np.cos(phi)).ravel()); ys.append((rho * np.sin(phi)).ravel())
+        zs.append(z.ravel()); ms.append((rho_bar * vol).ravel())
+    x, y, z, m = map(np.concatenate, (xs, ys, zs, ms))
+    m_core = float(ms[0].ravel()[0])
+    if eps_core is None:
+        eps_core = 0.05 * (m_core / rho_bar) ** (1.0 / 3.0)         # 1/20 of the core particle spacing
+    h = eps_core * np.cbrt(m / m_core)
+    w = Workload("stereographic_load", x, y, z, m, h, Lz=Lz, R_sim=R_sim, rho0=rho_bar)
+    w.cosmo.update(dict(rho_c=rho_c, omega_max=omega_max, n_core=int(ms[0].size), n_outer=int(ms[1].size),
+                        cells=(n_r, n_om, n_phi, n_z), m_core=m_core))
+    return w
+
+
 def make(config: int, n: int | None = None, seed: int | None = None) -> Workload:
     """The BASELINE.json config `config` (0..4), optionally at a reduced particle count."""
     gens = {0: uniform_cylinder, 1: compactified, 2: zeldovich, 3: lcdm_kdk, 4: clustered}

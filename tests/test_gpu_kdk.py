@@ -127,3 +127,37 @@ def test_free_streaming_conserves_a2v(torch_cuda):
         errs.append(float(np.abs(v[0].cpu().numpy() * a * a / (v0 * a0 * a0) - 1).max()))
         ctx.close()
     assert errs[0] < 1e-3 and errs[1] < errs[0] / 3.5
+
+
+def test_stereographic_load_parity_and_near_equilibrium(torch_cuda, oracle):
+    """The paper-faithful particle load (Eq. 21-22, Fig. 4 parameters, reduced N): parity of the pair sum
+    on sampled targets, and -- what the load is built for -- the pair sum is almost
+    cancelled by the homogeneous-cylinder term of Eq. 9 (exactly so only after glass-making)."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.stereographic_load(n_target=40000)
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=1.0, n_cut=5, R_sim=w.R_sim, rho0=w.rho0)
+    dev = [_dev(torch, a) for a in (w.x, w.y, w.z, w.m, w.h)]
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    bx, by = torch.empty_like(g[0]), torch.empty_like(g[0])
+    ctx.accel(*dev, *g)
+    ctx.background(dev[0], dev[1], bx, by)
+    ctx.check()
+    ctx.close()
+    gg = np.stack([t.cpu().numpy() for t in g], 1)
+    idx = workloads.sample_targets(w.n, 400, seed=6)
+    ref = np.stack(oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, 1.0, 5, targets=idx), 1)
+    e = np.linalg.norm(gg[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert e.max() <= 1e-10
+    net = gg.copy()
+    net[:, 0] += bx.cpu().numpy()
+    net[:, 1] += by.cpu().numpy()
+    rho = np.hypot(w.x, w.y)
+    inner = (rho > 20.0) & (rho < 0.8 * w.R_sim)          # away from the axis (|g| -> 0) and the edge
+    ratio = np.linalg.norm(net[inner], axis=1) / np.linalg.norm(gg[inner], axis=1)
+    assert np.median(ratio) < 0.25
+    # the radial part cancels on average (no systematic contraction / expansion)
+    gr = (gg[inner, 0] * w.x[inner] + gg[inner, 1] * w.y[inner]) / rho[inner]
+    nr = (net[inner, 0] * w.x[inner] + net[inner, 1] * w.y[inner]) / rho[inner]
+    assert abs(np.mean(nr)) < 0.03 * abs(np.mean(gr))
