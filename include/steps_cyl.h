@@ -55,13 +55,13 @@ typedef enum {
     STEPS_ESOFT        = -2,  /* softening precondition violated: some h_i <= 0 (or NaN)                   */
     STEPS_ECUDA        = -3,  /* a CUDA runtime call failed (or no device present)                     */
     STEPS_ENOMEM       = -4,  /* host or device allocation failed                                      */
-    STEPS_EUNSUPPORTED = -5   /* a combination this build does not contain (EWALD_TABLE with mixed
-                                 precision or with STEPS_FLAG_DETERMINISTIC)                           */
+    STEPS_EUNSUPPORTED = -5   /* a combination this build does not contain (EWALD_TABLE with
+                                 STEPS_FLAG_DETERMINISTIC, or a float table too large for shared memory) */
 } steps_cyl_status;
 
 enum { STEPS_PERIODIC_IMAGES = 0,      /* Eq. 8, truncated image sum                                  */
-       STEPS_PERIODIC_EWALD_TABLE = 1  /* Eq. 12-17: softened nearest image + interpolated table D;
-                                          fp64 precision only (mixed: STEPS_EUNSUPPORTED)              */ };
+       STEPS_PERIODIC_EWALD_TABLE = 1  /* Eq. 12-17: softened nearest image + interpolated table D
+                                          (mixed precision implies tab_fp32 = 1)                       */ };
 enum { STEPS_PREC_FP64 = 0,            /* every pair term and the accumulation in double               */
        STEPS_PREC_MIXED = 1            /* pair terms in float (cancellation-safe separations),
                                           accumulation over sources in double                          */ };

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsteps_cyl.so")
 SOURCES = [os.path.join(CSRC, "steps_cyl.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("pair_fp64.cuh", "pair_fp64_sym.cuh", "pair_mixed.cuh", "pair_mixed_sym.cuh", "pair_table_sym.cuh", "ewald_table.h", "aux_kernels.cuh")] \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("pair_fp64.cuh", "pair_fp64_sym.cuh", "pair_mixed.cuh", "pair_mixed_sym.cuh", "pair_table_sym.cuh", "pair_table_mixed_sym.cuh", "ewald_table.h", "aux_kernels.cuh")] \
     + [os.path.join(os.path.dirname(HERE), "include", "steps_cyl.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC",

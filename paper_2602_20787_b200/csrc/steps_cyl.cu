@@ -17,6 +17,7 @@
 #include "pair_mixed.cuh"
 #include "pair_mixed_sym.cuh"
 #include "pair_table_sym.cuh"
+#include "pair_table_mixed_sym.cuh"
 #include "ewald_table.h"
 
 using namespace steps;
@@ -40,7 +41,8 @@ struct steps_cyl_ctx {
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
     float2 *d_table_f32 = nullptr;                 // the same rounded to float (tab_fp32), staged in smem
-    size_t table_smem_bytes = 0;
+    size_t table_smem_bytes = 0, table_mixed_smem_bytes = 0;
+    TableConstsF32 tcf;
     TableConsts tc;
     bool table_mode = false;
     int n_nodes = 0;
@@ -157,7 +159,17 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
     if (c->table_mode) {
         dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
         const size_t sb4 = 4 * 3 * PAIR_THREADS * sizeof(double);
-        if (c->d_table_f32) {
+        if (c->p.precision == STEPS_PREC_MIXED) {
+            dim3 g16(c->n_tiles / (4 * SYM_R), c->sym_chunks);
+            if (c->tc.interp == STEPS_INTERP_CIC)
+                pair_table_mixed_sym_kernel<0><<<g16, 512, c->table_mixed_smem_bytes, s>>>(
+                    c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->mc,
+                    c->tcf, c->d_table_f32, c->part);
+            else
+                pair_table_mixed_sym_kernel<1><<<g16, 512, c->table_mixed_smem_bytes, s>>>(
+                    c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->mc,
+                    c->tcf, c->d_table_f32, c->part);
+        } else if (c->d_table_f32) {
             dim3 g16(c->n_tiles / (4 * SYM_R), c->sym_chunks);
             if (c->tc.interp == STEPS_INTERP_CIC)
                 pair_table_sym_kernel<0, 16, true><<<g16, 512, c->table_smem_bytes, s>>>(
@@ -274,8 +286,8 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             !(pp.tab_rho_max > 0.0) || !std::isfinite(pp.tab_rho_max) ||
             (pp.interp != STEPS_INTERP_CIC && pp.interp != STEPS_INTERP_TSC))
             return STEPS_EINVAL;
-        if (p->precision != STEPS_PREC_FP64 || (p->flags & STEPS_FLAG_DETERMINISTIC))
-            return STEPS_EUNSUPPORTED;
+        if (p->flags & STEPS_FLAG_DETERMINISTIC) return STEPS_EUNSUPPORTED;
+        if (p->precision == STEPS_PREC_MIXED) pp.tab_fp32 = 1;      // mixed mode always uses the float table
     }
 
     steps_cyl_ctx *ctx = new (std::nothrow) steps_cyl_ctx();
@@ -368,6 +380,15 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             for (size_t q = 0; q < nodes * 2; ++q) Df[q] = (float)D[q];
             A(dev_alloc(&ctx->d_table_f32, nodes));
             if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table_f32, Df.data(), nodes * sizeof(float2), cudaMemcpyHostToDevice));
+            ctx->table_mixed_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(float) + nodes * sizeof(float2);
+            ctx->tcf.nrho = pp.tab_nrho;
+            ctx->tcf.nz = pp.tab_nz;
+            ctx->tcf.rho_max2 = (float)(pp.tab_rho_max * pp.tab_rho_max);
+            ctx->tcf.inv_drho = (float)((double)(pp.tab_nrho - 1) / pp.tab_rho_max);
+            ctx->tcf.inv_dz = (float)((double)(pp.tab_nz - 1) / (0.5 * pp.Lz));
+            ctx->tcf.two_over_L = (float)(2.0 / pp.Lz);
+            A(cudaFuncSetAttribute(pair_table_mixed_sym_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_mixed_sym_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
             A(cudaFuncSetAttribute(pair_table_sym_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
             A(cudaFuncSetAttribute(pair_table_sym_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
             if (rc != STEPS_OK) return fail(rc);
@@ -604,7 +625,7 @@ const char *steps_cyl_strerror(int code)
     case STEPS_ESOFT: return "softening precondition violated (some h_i <= 0)";
     case STEPS_ECUDA: return "CUDA runtime error (see steps_cyl_last_cuda_error)";
     case STEPS_ENOMEM: return "out of memory";
-    case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE needs fp64 and no DETERMINISTIC flag)";
+    case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE with the DETERMINISTIC flag, or a float table too large for shared memory)";
     default: return "unknown status";
     }
 }

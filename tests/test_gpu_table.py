@@ -120,3 +120,20 @@ def test_table_mode_fp32_table_in_shared_memory(torch_cuda, oracle, interp):
     # and the float table changes the answer itself only at the 1e-8 level
     ref64 = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, interp)
     assert rel_err(g, ref64).max() <= 1e-6
+
+
+@pytest.mark.parametrize("interp", [0, 1])
+def test_table_mode_mixed_precision(torch_cuda, oracle, interp):
+    """EWALD_TABLE in mixed precision (float pair terms and float interpolation of the shared-memory
+    float table, double accumulation across rings): the mixed-mode bar, RMS <= 1e-5 and max <= 1e-4."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    for cfg, n in [(1, 9000), (4, 12000)]:
+        w = workloads.make(cfg, n=n)
+        rmax = 5.0 * w.Lz
+        D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, 144, 128, rmax).astype(np.float32).astype(np.float64)
+        ref = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, interp)
+        g = gpu_accel_table(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, interp=interp,
+                            precision=b.PREC_MIXED)
+        e = rel_err(g, ref)
+        assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4, (e.max(), np.sqrt(np.mean(e ** 2)))
