@@ -45,6 +45,9 @@ KERNEL_MIX = {
     # unordered pair per iteration; independent of n_cut
     "table": dict(kernel="pair_table_sym_kernel<CIC>", interactions=2, dfma=22, dmul=14, dadd=14, dsetp=5,
                   per_image=(0.0, 0.0)),
+    # --periodic table --precision mixed: pair_table_mixed_sym_kernel<CIC>, one unordered pair per iteration
+    "mixed_table": dict(kernel="pair_table_mixed_sym_kernel<CIC>", interactions=2, ffma=18, fmul=11, fadd=19,
+                        mufu=2, f2f=2, dadd=0),
     # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
     # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
     "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=25, fmul=24, fadd=29, mufu=10,
@@ -65,7 +68,7 @@ def pipe_counts(mode, n_cut):
     if mode.startswith("mixed"):
         instr = mix["ffma"] + mix["fmul"] + mix["fadd"]
         flops = 2 * mix["ffma"] + mix["fmul"] + mix["fadd"]
-        d = 2 * (n_cut - 5)
+        d = 0 if mode == "mixed_table" else 2 * (n_cut - 5)
         return (instr + 7.5 * d) / mix["interactions"], (flops + 9.0 * d) / mix["interactions"]
     instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
     flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
@@ -302,7 +305,10 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peaks_kind = load_peaks()
-    mode = "table" if table else ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
+    if table:
+        mode = "mixed_table" if prec == b.PREC_MIXED else "table"
+    else:
+        mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
     instr, flops = pipe_counts(mode, args.n_cut)
     t_pair = float(np.mean(pair_ms)) * 1e-3
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
@@ -323,7 +329,8 @@ def run_ours(args):
     }
     if is_mixed:
         xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
-        mufu = (2 * args.n_cut + KERNEL_MIX[mode]["f2f"]) / KERNEL_MIX[mode]["interactions"]
+        mufu = ((KERNEL_MIX[mode]["mufu"] if table else 2 * args.n_cut) + KERNEL_MIX[mode]["f2f"]) \
+            / KERNEL_MIX[mode]["interactions"]
         roofline["xu_pipe_util_vs_nominal"] = mufu * pairs_per_step / t_pair / xu_peak
     else:
         roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
@@ -339,7 +346,7 @@ def run_ours(args):
                "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
                          "%.1f s" % (len(idx), n, tc)}
     periodic_desc = ("Ewald table 144x128 CIC%s, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10"
-                     % (" (float nodes in shared memory)" if args.table_fp32 else "") if table
+                     % (" (float nodes in shared memory)" if (args.table_fp32 or prec == b.PREC_MIXED) else "") if table
                      else "n_cut=%d (%d images/pair), background Eq. 9" % (args.n_cut, 2 * args.n_cut))
     line = {
         "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
