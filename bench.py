@@ -60,6 +60,7 @@ METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
 NOMINAL_FP64_LANES_PER_SM = 64
 NOMINAL_FP32_LANES_PER_SM = 128
 NOMINAL_XU_LANES_PER_SM = 16
+NCU_DRAM_BYTES_DEFAULT = 78.49e6 + 8.60e6     # pair_fp64_sym_kernel<5>, N = 1 048 576 (algorithmic: 42 MB + 34 MB)
 
 
 def pipe_counts(mode, n_cut):
@@ -320,7 +321,11 @@ def run_ours(args):
     roofline = {
         "bound": "alu", "kernel": KERNEL_MIX[mode]["kernel"].replace("<5", "<%d" % args.n_cut),
         "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
-        "frac": achieved_tflops / nominal_tflops, "traffic": None,
+        "frac": achieved_tflops / nominal_tflops,
+        # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one `ncu --set full` capture of the
+        # default configuration (profiles/r1_ncu_full_pair_kernels.md); other configurations: not captured
+        "traffic": NCU_DRAM_BYTES_DEFAULT if (mode == "fp64" and n == 1048576 and args.n_cut == 5) else None,
+        "traffic_unit": "bytes per launch (ncu); the bound is the FP64 pipe, not HBM",
         "peak_kind": "nominal %s FMA: %d SMs x %d lanes x 2 flop x %.0f MHz (DESIGN.md)"
                      % ("FP32" if is_mixed else "FP64", sm_count, lanes, sm_max),
         "flops_per_pair_interaction": flops, "pipe_instr_per_pair_interaction": instr,
