@@ -50,7 +50,9 @@ KERNEL_MIX = {
                         mufu=2, f2f=2, dadd=0),
     # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
     # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
-    "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=25, fmul=24, fadd=29, mufu=10,
+    # (main loop: 38 FFMA2 + 19 FMUL2 + 16 FADD2 + 20 MUFU per ring step of two unordered pairs; counted
+    # here as scalar FP32 operations per unordered pair)
+    "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=38, fmul=19, fadd=16, mufu=10,
                   f2f=0, dadd=0),
     # STEPS_FLAG_DETERMINISTIC, pair_mixed_kernel<5>: one ordered pair per iteration
     "mixed_det": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,

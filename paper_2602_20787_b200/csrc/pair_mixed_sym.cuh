@@ -114,9 +114,138 @@ __device__ __forceinline__ void ring_subtile_f32(const MixTgt (&ti)[R], const in
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Packed path: sm_100 has two-wide FP32 instructions (PTX add/sub/mul/fma .f32x2 -> SASS FADD2 /
+// FMUL2 / FFMA2, scalar operands broadcast for free).  The kernel is bound by instruction issue, and
+// the two targets a lane holds go through identical arithmetic against the same source, so they are
+// processed as the two halves of one packed value: half the FP32 instructions per pair.  MUFU.RSQ
+// (one per image per target), the compares and the sign / mask bit operations stay scalar.
+#ifndef STEPS_MIXED_UNROLL
+#define STEPS_MIXED_UNROLL 1
+#endif
+#ifndef STEPS_MIXED_MINBLOCKS
+#define STEPS_MIXED_MINBLOCKS 4
+#endif
+constexpr int kMixedUnroll = STEPS_MIXED_UNROLL;
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk(float2 a) { return *reinterpret_cast<u64 *>(&a); }
+__device__ __forceinline__ float2 upk(u64 a) { return *reinterpret_cast<float2 *>(&a); }
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
+{
+    u64 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b)
+{
+    u64 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b)
+{
+    u64 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    u64 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 rsqrt2(float2 x) { return make_float2(rsqrt_f32(x.x), rsqrt_f32(x.y)); }
+__device__ __forceinline__ float2 cube2(float2 y) { return mul2(mul2(y, y), y); }
+
+struct MixTgt2 { float2 xh, yh, zh, xl, yl, zl, h, m, mL; };       // .x: target tile r = 0, .y: r = 1
+
+// 32 ring steps, both targets of the lane at once, symmetric (source side accumulated too).
+// a[c] (c = 0..3: A_x, A_y, A_z1, A_z2) and bx, by, bz are FLOAT partial sums of this ring, the two
+// halves belonging to the two targets; the caller adds the halves of b.
+template <int NC>
+__device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int (&soft_bits)[2],
+                                                   const float4 *s_hi, const float4 *s_lo, int lane,
+                                                   const MixedConsts &k, int ncut_rt, float2 (&a)[4],
+                                                   float2 &bx, float2 &by, float2 &bz)
+{
+    bx = by = bz = bc(0.0f);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) a[c] = bc(0.0f);
+    const float invL = 1.0f / k.Lh, magic = 12582912.0f;          // 1.5 * 2^23: round-to-nearest-integer
+#pragma unroll kMixedUnroll
+    for (int s = 0; s < 32; ++s) {
+        const int jj = (lane + s) & 31;
+        const float4 jh = s_hi[jj], jl = s_lo[jj];          // {x_hi,y_hi,z_hi,m}, {x_lo,y_lo,z_lo,h}
+        const float2 rx = add2(sub2(ti.xh, bc(jh.x)), sub2(ti.xl, bc(jl.x)));
+        const float2 ry = add2(sub2(ti.yh, bc(jh.y)), sub2(ti.yl, bc(jl.y)));
+        float2 rzh = sub2(ti.zh, bc(jh.z)), rzl = sub2(ti.zl, bc(jl.z));
+        // nearest image: k = rint(rz / L) by the magic-number trick (|rz| < L, so k in {-1, 0, 1});
+        // a tie at |rz| = L/2 may go either way (the image set is symmetric then)
+        const float2 kk = sub2(fma2(rzh, bc(invL), bc(magic)), bc(magic));
+        rzh = fma2(kk, bc(-k.Lh), rzh);
+        rzl = fma2(kk, bc(-k.Ll), rzl);
+        const float2 rz = add2(rzh, rzl);
+        const float2 rho2 = fma2(ry, ry, mul2(rx, rx));
+        const float2 q = fma2(rz, rz, rho2);
+        float2 w0 = cube2(rsqrt2(q));
+        if (__float_as_int(q.x) <= soft_bits[0] || __float_as_int(q.y) <= soft_bits[1]) {
+            const float h0 = ti.h.x + jl.w, h1 = ti.h.y + jl.w;
+            if (q.x < h0 * h0) w0.x = spline_w_f32(q.x, h0);
+            if (q.y < h1 * h1) w0.y = spline_w_f32(q.y, h1);
+        }
+        float2 S = w0, T = bc(0.0f);
+        const int n_img = (NC > 0) ? NC : ncut_rt;
+        if (NC > 0) {
+#pragma unroll
+            for (int n = 1; n < NC; ++n) {
+                const float2 B  = add2(q, bc(k.n2L2[n]));
+                const float2 wp = cube2(rsqrt2(fma2(bc(-k.c2nL[n]), rz, B)));
+                const float2 wm = cube2(rsqrt2(fma2(bc(k.c2nL[n]), rz, B)));
+                S = add2(add2(S, wp), wm);
+                T = (n == 1) ? sub2(wp, wm) : fma2(bc((float)n), sub2(wp, wm), T);
+            }
+        } else {
+            for (int n = 1; n < ncut_rt; ++n) {
+                const float nL = (float)n * k.Lh;
+                const float2 B  = fma2(bc(nL), bc(nL), q);
+                const float2 wp = cube2(rsqrt2(fma2(bc(-2.0f * nL), rz, B)));
+                const float2 wm = cube2(rsqrt2(fma2(bc(2.0f * nL), rz, B)));
+                S = add2(add2(S, wp), wm);
+                T = fma2(bc((float)n), sub2(wp, wm), T);
+            }
+        }
+        {   // end image n = sign(rz) N_cut, absent when rz == 0
+            const float NL = (float)n_img * k.Lh;
+            const float2 arz = make_float2(fabsf(rz.x), fabsf(rz.y));
+            const float2 Be = (NC > 0) ? add2(q, bc(k.n2L2[NC > 0 ? NC : 0])) : fma2(bc(NL), bc(NL), q);
+            float2 we = cube2(rsqrt2(fma2(bc(-2.0f * NL), arz, Be)));
+            we.x = (rz.x == 0.0f) ? 0.0f : we.x;
+            we.y = (rz.y == 0.0f) ? 0.0f : we.y;
+            S = add2(S, we);
+            const float2 ns = make_float2(copysignf((float)n_img, rz.x), copysignf((float)n_img, rz.y));
+            T = fma2(ns, we, T);
+        }
+        const float2 Sj = mul2(bc(jh.w), S);
+        a[0] = fma2(Sj, rx, a[0]);
+        a[1] = fma2(Sj, ry, a[1]);
+        a[2] = fma2(Sj, rz, a[2]);
+        a[3] = fma2(bc(jh.w), T, a[3]);
+        const float2 Si = mul2(ti.m, S);
+        bx = fma2(Si, rx, bx);
+        by = fma2(Si, ry, by);
+        bz = fma2(Si, rz, bz);
+        bz = fma2(ti.mL, T, bz);
+        const int src = (lane + 1) & 31;
+        bx = upk(__shfl_sync(0xffffffffu, pk(bx), src));
+        by = upk(__shfl_sync(0xffffffffu, pk(by), src));
+        bz = upk(__shfl_sync(0xffffffffu, pk(bz), src));
+    }
+}
+
 // Same grid / decomposition / acc layout as pair_fp64_sym_kernel.
 template <int NC>
-__global__ void __launch_bounds__(PAIR_THREADS, 4)
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
 pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
                       const double *__restrict__ tile_hmax, int n_pad, int n_tiles,
                       int tiles_per_chunk, int ncut_rt, MixedConsts k, double halfL,
@@ -146,6 +275,13 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
         ti[r].mL = -k.Lh * h4.w;
         A[r][0] = A[r][1] = A[r][2] = A[r][3] = 0.0;
     }
+    static_assert(SYM_R == 2, "the packed path holds exactly two targets per lane");
+    MixTgt2 ti2;
+    ti2.xh = make_float2(ti[0].xh, ti[1].xh); ti2.yh = make_float2(ti[0].yh, ti[1].yh);
+    ti2.zh = make_float2(ti[0].zh, ti[1].zh); ti2.xl = make_float2(ti[0].xl, ti[1].xl);
+    ti2.yl = make_float2(ti[0].yl, ti[1].yl); ti2.zl = make_float2(ti[0].zl, ti[1].zl);
+    ti2.h = make_float2(ti[0].h, ti[1].h);    ti2.m = make_float2(ti[0].m, ti[1].m);
+    ti2.mL = make_float2(ti[0].mL, ti[1].mL);
 
     for (int t = t0; t < t1; ++t) {
         const int j = t * PAIR_THREADS + threadIdx.x;
@@ -167,12 +303,16 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
             float bx = 0.0f, by = 0.0f, bz = 0.0f;
             const float4 *sh = s_hi + js * 32, *sl = s_lo + js * 32;
             if (t >= tb + SYM_R) {
-                float a[SYM_R][4];
-                ring_subtile_f32<NC, SYM_R, true>(ti, soft_bits, sh, sl, lane, k, ncut_rt, a, bx, by, bz);
+                float2 a2[4], b2x, b2y, b2z;
+                ring_subtile_f32x2<NC>(ti2, soft_bits, sh, sl, lane, k, ncut_rt, a2, b2x, b2y, b2z);
 #pragma unroll
-                for (int r = 0; r < SYM_R; ++r)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) A[r][c] += (double)a[r][c];
+                for (int c = 0; c < 4; ++c) {
+                    A[0][c] += (double)a2[c].x;
+                    A[1][c] += (double)a2[c].y;
+                }
+                bx = b2x.x + b2x.y;
+                by = b2y.x + b2y.y;
+                bz = b2z.x + b2z.y;
             } else {
 #pragma unroll
                 for (int r = 0; r < SYM_R; ++r) {
