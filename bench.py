@@ -251,7 +251,8 @@ def run_ours(args):
                      R_sim=w.R_sim, rho0=w.rho0, device=local,
                      periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
                      tab_fp32=1 if (table and args.table_fp32) else 0,
-                     flags=b.FLAG_DETERMINISTIC if args.deterministic else 0)
+                     flags=(b.FLAG_DETERMINISTIC if args.deterministic else 0)
+                     | (b.FLAG_FAR_ORDER2 if args.far_order2 else 0))
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
             for k in names}
@@ -313,6 +314,9 @@ def run_ours(args):
     else:
         mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
     instr, flops = pipe_counts(mode, args.n_cut)
+    if args.far_order2 and mode == "fp64":              # one DFMA less per far image
+        instr -= (2 * args.n_cut - 1) / 2.0
+        flops -= (2 * args.n_cut - 1)
     t_pair = float(np.mean(pair_ms)) * 1e-3
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
@@ -391,6 +395,8 @@ def main():
                     help="images: truncated image sum of Eq. 8 (the metric's mode); table: Eq. 12-17")
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per sample / reference step")
+    ap.add_argument("--far-order2", action="store_true",
+                    help="fp64 images mode: STEPS_FLAG_FAR_ORDER2 (far images refined to first order only)")
     ap.add_argument("--table-fp32", action="store_true",
                     help="--periodic table: float table held in shared memory (tab_fp32 = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -74,7 +74,10 @@ enum { STEPS_FLAG_DETERMINISTIC = 1    /* fp64 mode: evaluate every ORDERED pair
                                           order (bit-reproducible, ~1.9x slower) instead of the default
                                           kernel, which evaluates every unordered pair once and applies
                                           it to both particles with floating-point atomics (same terms,
-                                          summation order varies from run to run)                      */ };
+                                          summation order varies from run to run)                      */
+       STEPS_FLAG_FAR_ORDER2 = 2       /* fp64 images mode, default kernel only: the rsqrt refinement of
+                                          the FAR images (n != 0) drops its second-order term: 8 % faster,
+                                          per-particle error ~3e-12 instead of ~1e-14 (bar: 1e-10)     */ };
 
 typedef struct steps_cyl_ctx steps_cyl_ctx;   /* opaque; created by init, freed by destroy */
 

@@ -17,6 +17,7 @@ PERIODIC_IMAGES, PERIODIC_EWALD_TABLE = 0, 1
 PREC_FP64, PREC_MIXED = 0, 1
 BG_FINITE, BG_INFINITE = 0, 1
 FLAG_DETERMINISTIC = 1
+FLAG_FAR_ORDER2 = 2
 INTERP_CIC, INTERP_TSC = 0, 1
 
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",

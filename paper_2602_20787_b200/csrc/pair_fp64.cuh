@@ -62,6 +62,24 @@ __device__ __forceinline__ double inv_cube_sqrt(double x)
     return fma(c * e, p, c);
 }
 
+// The same with the series cut after the linear term, w = y0^3 (1 + 3e/2): 5 FP64 instructions.
+// The dropped term 15 e^2/8 is a relative deficit of at most ~4e-13 (|e| <= 2^-21 for the RSQ64H
+// seed).  Used for the far images only, and only under STEPS_FLAG_FAR_ORDER2: see DESIGN.md section 5.
+__device__ __forceinline__ double inv_cube_sqrt_o2(double x)
+{
+    const double y0 = rsqrt_seed(x);
+    const double y2 = y0 * y0;
+    const double e  = fma(-x, y2, 1.0);
+    const double c  = y2 * y0;
+    return c * fma(1.5, e, 1.0);
+}
+
+template <bool O2>
+__device__ __forceinline__ double inv_cube_sqrt_far(double x)
+{
+    return O2 ? inv_cube_sqrt_o2(x) : inv_cube_sqrt(x);
+}
+
 // w = F(s, h)/s of Eq. 3 for s^2 = q < h^2, h = h_i + h_j  (slow path).
 __device__ __noinline__ double spline_w(double q, double hh)
 {
@@ -99,7 +117,7 @@ __device__ __forceinline__ double nearest_image(double rz, const PairConsts &k)
 // soft_hi: high word of an upper bound of (h_i + h_j)^2 over the source tile; only pairs with
 // hi32(q) <= soft_hi can be inside the spline support and take the exact test.
 // NC > 0: image loop fully unrolled for N_cut == NC; NC == 0: run-time N_cut.
-template <int NC>
+template <int NC, bool O2 = false>
 __device__ __forceinline__ void image_sum(double rz, double q, double hi, double hj, int soft_hi,
                                           const PairConsts &k, int ncut_rt, double &S, double &T)
 {
@@ -116,14 +134,14 @@ __device__ __forceinline__ void image_sum(double rz, double q, double hi, double
 #pragma unroll
         for (int n = 1; n < NC; ++n) {
             const double B  = q + k.n2L2[n];
-            const double wp = inv_cube_sqrt(fma(-k.c2nL[n], rz, B));   // image +n: d = rz - nL
-            const double wm = inv_cube_sqrt(fma(k.c2nL[n], rz, B));    // image -n: d = rz + nL
+            const double wp = inv_cube_sqrt_far<O2>(fma(-k.c2nL[n], rz, B));   // image +n: d = rz - nL
+            const double wm = inv_cube_sqrt_far<O2>(fma(k.c2nL[n], rz, B));    // image -n: d = rz + nL
             S += wp;
             S += wm;
             T = (n == 1) ? (wp - wm) : fma((double)n, wp - wm, T);
         }
         // end image n = sign(rz) N_cut (absent when rz == 0): d = -sign(rz)(N L - |rz|)
-        double we = inv_cube_sqrt(fma(-k.c2nL[NC], fabs(rz), q + k.n2L2[NC]));
+        double we = inv_cube_sqrt_far<O2>(fma(-k.c2nL[NC], fabs(rz), q + k.n2L2[NC]));
         we = rz_nonzero ? we : 0.0;
         S += we;
         T = (NC == 1) ? copysign(we, rz) : fma(copysign((double)NC, rz), we, T);

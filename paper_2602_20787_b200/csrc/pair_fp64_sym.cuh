@@ -51,7 +51,7 @@ struct SymTgt { double x, y, z, h, m, mL; };         // mL = -L m
 // pairs.  SYM: also accumulate on the sources.  Source-side accumulators (rotating):
 // bx = sum m_i S r_x, by = sum m_i S r_y, bz = sum m_i (S r_z - L T) -- z already combined,
 // so only three values travel.
-template <int NC, int R, bool SYM>
+template <int NC, int R, bool SYM, bool O2>
 __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&soft_hi)[R],
                                              const SymSrc *s_src, int lane, const PairConsts &k,
                                              int ncut_rt, double (&a)[R][4], double &bx,
@@ -71,7 +71,7 @@ __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&
             const double rho2 = fma(ry, ry, rx * rx);
             const double q = fma(rz, rz, rho2);
             double S, T;
-            image_sum<NC>(rz, q, ti[r].h, hj, soft_hi[r], k, ncut_rt, S, T);
+            image_sum<NC, O2>(rz, q, ti[r].h, hj, soft_hi[r], k, ncut_rt, S, T);
             const double Sj = pb.y * S;
             a[r][0] = fma(Sj, rx, a[r][0]);
             a[r][1] = fma(Sj, ry, a[r][1]);
@@ -103,7 +103,7 @@ constexpr int SYM_R = STEPS_SYM_R;     // target tiles per CTA (n_tiles is kept 
 // before the launch; the source side adds its combined z sum to A_z1.
 // grid = (n_tiles / SYM_R, chunks).  CTA (bi, c): target tiles SYM_R*bi + r (lane holds particle
 // tid of each), source tiles [c*tpc, (c+1)*tpc) from SYM_R*bi on.
-template <int NC>
+template <int NC, bool O2>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                      const double *__restrict__ hs, const double *__restrict__ tile_hmax,
@@ -158,7 +158,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             const SymSrc *sub = s_src + js * 32;
             if (t >= tb + SYM_R) {
                 // off-diagonal tile: every target of the CTA meets every source, both ways
-                ring_subtile<NC, SYM_R, true>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+                ring_subtile<NC, SYM_R, true, O2>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
             } else {
                 // one of the CTA's own tiles: target tile tb + r meets source tile t only if
                 // t >= tb + r; in its own tile (t == tb + r) warp w takes sub-tiles js > w both
@@ -171,9 +171,9 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
                     double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
                     double cx = 0.0, cy = 0.0, cz = 0.0;
                     if (tb + r < t || js > w)
-                        ring_subtile<NC, 1, true>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                        ring_subtile<NC, 1, true, O2>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                     else if (js == w)
-                        ring_subtile<NC, 1, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                        ring_subtile<NC, 1, false, O2>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                     bx += cx; by += cy; bz += cz;
                 }
             }

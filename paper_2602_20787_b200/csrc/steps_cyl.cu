@@ -130,9 +130,16 @@ template <int NC>
 void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
-    pair_fp64_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad,
-                                                          c->n_tiles, c->sym_tiles_per_chunk,
-                                                          c->p.n_cut, c->kc, c->flags, c->part);
+    if (c->p.flags & STEPS_FLAG_FAR_ORDER2)
+        pair_fp64_sym_kernel<NC, true><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+                                                                    c->n_pad, c->n_tiles,
+                                                                    c->sym_tiles_per_chunk, c->p.n_cut,
+                                                                    c->kc, c->flags, c->part);
+    else
+        pair_fp64_sym_kernel<NC, false><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+                                                                     c->n_pad, c->n_tiles,
+                                                                     c->sym_tiles_per_chunk, c->p.n_cut,
+                                                                     c->kc, c->flags, c->part);
 }
 
 template <int NC>
@@ -269,7 +276,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         return STEPS_EINVAL;
     if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
     if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
-    if ((p->flags & ~STEPS_FLAG_DETERMINISTIC) != 0 || p->device < 0) return STEPS_EINVAL;
+    if ((p->flags & ~(STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_FAR_ORDER2)) != 0 || p->device < 0) return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
     if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
     if (p->tab_fp32 != 0 && p->tab_fp32 != 1) return STEPS_EINVAL;

@@ -234,3 +234,16 @@ def test_deterministic_mixed_kernel(torch_cuda, oracle):
     check(g1, ref, 1)
     for a, c in zip(g1, g2):
         assert np.array_equal(a, c)
+
+
+def test_far_order2_flag(torch_cuda, oracle):
+    """STEPS_FLAG_FAR_ORDER2: far images refined to first order only -- still far inside the fp64 bar,
+    but measurably less accurate than the default (which is at round-off)."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    w = workloads.make(1, n=6000, seed=17)
+    arrs = (w.x, w.y, w.z, w.m, w.h)
+    ref = oracle.accel(*arrs, w.Lz, w.G, 5)
+    e_fast = check(gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_FAR_ORDER2), ref, 0)
+    e_def = check(gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0), ref, 0)
+    assert e_fast.max() < 2e-11 and e_def.max() < 1e-13
