@@ -70,7 +70,7 @@ enum { STEPS_INTERP_CIC = 0,           /* cloud-in-cell: bilinear in (rho, z)   
 enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz                                    */
        STEPS_BG_INFINITE = 1           /* Eq. 10                                                       */ };
 
-enum { STEPS_FLAG_DETERMINISTIC = 1    /* fp64 mode: evaluate every ORDERED pair and reduce in a fixed
+enum { STEPS_FLAG_DETERMINISTIC = 1,   /* fp64 mode: evaluate every ORDERED pair and reduce in a fixed
                                           order (bit-reproducible, ~1.9x slower) instead of the default
                                           kernel, which evaluates every unordered pair once and applies
                                           it to both particles with floating-point atomics (same terms,
