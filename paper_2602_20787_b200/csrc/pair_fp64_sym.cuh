@@ -9,18 +9,19 @@
 //     target j :  A_j -= m_i (S r_x, S r_y, S r_z, T)
 // which nearly halves the FP64-pipe work per ordered pair interaction.
 //
-// Mapping (no cross-lane reduction anywhere): a warp owns 32 targets i (one per lane, in
-// registers) and walks a 32-source sub-tile as a ring: at step s lane l meets source
-// (l + s) mod 32, whose data it reads from the shared-memory tile and whose accumulator is in
-// lane l's registers; after the step the four source accumulators move one lane down
-// (6 SHFL), so that after 32 steps every accumulator is back in its home lane and has met all
-// 32 targets.  Home accumulators go to a per-warp shared slab, the four slabs of the CTA are
-// summed at the end of the tile and leave with one RED.ADD.F64 per value.
+// Mapping (no cross-lane reduction anywhere): a lane holds SYM_R = 2 targets in registers (one from
+// each of the CTA's two target tiles), and its warp walks a 32-source sub-tile as a ring: at step
+// s lane l meets source (l + s) mod 32, whose record it reads from the shared-memory tile and
+// whose three accumulators (sum m_i S r_x, sum m_i S r_y, sum m_i (S r_z - L T)) are in lane l's
+// registers; after the step they move one lane down (6 SHFL), so that after 32 steps every
+// accumulator is back in its home lane having met all 2 x 32 targets of the warp.  Home
+// accumulators go to a per-warp shared slab; the four slabs of the CTA are summed at the end of the
+// tile and leave with one RED.ADD.F64 per value.
 //
-// Work decomposition: CTA (bi, c) = target block bi x source tiles [c*tpc, (c+1)*tpc) with
-// tile >= bi (upper triangle).  In the diagonal tile, warp w takes sub-tiles js > w both ways,
-// js == w target-side only (every ordered pair of the 32x32 block once; j == i contributes
-// exactly 0), and skips js < w.
+// Work decomposition: CTA (b, c) = target tiles 2b, 2b+1 x source tiles [c*tpc, (c+1)*tpc) from 2b
+// on (upper triangle).  In one of its own tiles, target tile tt meets source tile t only if
+// t >= tt; for t == tt warp w takes sub-tiles js > w both ways, js == w target-side only (every
+// ordered pair of the 32 x 32 block once; j == i contributes exactly 0), and skips js < w.
 //
 // Results are accumulated with floating-point atomics, so the summation ORDER (not the set of
 // terms) can differ from run to run: results are reproducible to round-off (~1e-16 relative),
