@@ -247,3 +247,34 @@ def test_far_order2_flag(torch_cuda, oracle):
     e_fast = check(gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_FAR_ORDER2), ref, 0)
     e_def = check(gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0), ref, 0)
     assert e_fast.max() < 2e-11 and e_def.max() < 1e-13
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_randomised_parameters(torch_cuda, oracle, seed):
+    """Seeded random problem set-ups: period not representable in float, length scales from 1e-2 to
+    1e4, either sign of G, masses over three decades, softenings up to the point where the general
+    path takes over, z far outside [0, L), clustered and diffuse particles mixed."""
+    rng = np.random.default_rng(4000 + seed)
+    L = float(rng.choice([1.0, 77.7, 0.0123, 1.0e4, 100.0 / 3.0]))
+    n = int(rng.integers(100, 2500))
+    n_cut = int(rng.integers(1, 10))
+    G = float(rng.choice([1.0, -0.37, 4.30091e-9, 6.5]))
+    R = L * float(rng.choice([0.3, 2.0, 15.0]))
+    r = R * rng.random(n) ** float(rng.choice([0.5, 2.0]))
+    phi = 2 * np.pi * rng.random(n)
+    x, y = r * np.cos(phi), r * np.sin(phi)
+    z = L * (rng.random(n) * 7.0 - 3.0)                       # several periods either side
+    k = n // 5                                                # a tight clump: softened pairs
+    x[:k] = x[0] + 0.01 * L * rng.normal(size=k)
+    y[:k] = y[0] + 0.01 * L * rng.normal(size=k)
+    z[:k] = z[0] + 0.01 * L * rng.normal(size=k)
+    m = 10.0 ** rng.uniform(-1.5, 1.5, n)
+    hmax = L * float(rng.choice([0.002, 0.05, 0.12, 0.4]))    # 0.4 L: 2 hmax > L/2 -> general path
+    h = hmax * rng.uniform(0.2, 1.0, n)
+    ref = oracle.accel(x, y, z, m, h, L, G, n_cut)
+    general = 2 * h.max() > L / 2
+    for precision in (0, 1):
+        g = gpu_accel(torch_cuda, (x, y, z, m, h), L, G, n_cut, precision)
+        check(g, ref, 0 if general else precision)
+    g = gpu_accel(torch_cuda, (x, y, z, m, h), L, G, n_cut, 0, flags=1)
+    check(g, ref, 0)

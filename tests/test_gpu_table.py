@@ -137,3 +137,37 @@ def test_table_mode_mixed_precision(torch_cuda, oracle, interp):
                             precision=b.PREC_MIXED)
         e = rel_err(g, ref)
         assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4, (e.max(), np.sqrt(np.mean(e ** 2)))
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_table_mode_randomised_parameters(torch_cuda, oracle, seed):
+    rng = np.random.default_rng(7000 + seed)
+    L = float(rng.choice([1.0, 77.7, 1.0e3]))
+    n = int(rng.integers(200, 2500))
+    G = float(rng.choice([1.0, -0.37, 6.5]))
+    R = L * float(rng.choice([0.5, 3.0, 9.0]))
+    r = R * np.sqrt(rng.random(n))
+    phi = 2 * np.pi * rng.random(n)
+    x, y = r * np.cos(phi), r * np.sin(phi)
+    z = L * (rng.random(n) * 5.0 - 2.0)
+    m = 10.0 ** rng.uniform(-1.0, 1.0, n)
+    h = L * 0.05 * rng.uniform(0.2, 1.0, n)
+    nrho, nz = int(rng.integers(20, 60)), int(rng.integers(17, 50))
+    rmax = L * float(rng.choice([2.0, 4.0]))
+    alpha = float(rng.choice([1.5, 2.0, 3.0])) / L
+    interp = int(rng.integers(0, 2))
+    D = oracle.ewald_table(L, alpha, 5, 12, nrho, nz, rmax)
+    ref = oracle.accel_table(x, y, z, m, h, L, G, D, rmax, interp)
+    g = gpu_accel_table(torch_cuda, (x, y, z, m, h), L, G, tab_nrho=nrho, tab_nz=nz, tab_rho_max=rmax,
+                        interp=interp, ew_alpha=alpha)
+    assert rel_err(g, ref).max() <= 1e-10
+    D32 = D.astype(np.float32).astype(np.float64)
+    ref32 = oracle.accel_table(x, y, z, m, h, L, G, D32, rmax, interp)
+    g = gpu_accel_table(torch_cuda, (x, y, z, m, h), L, G, tab_nrho=nrho, tab_nz=nz, tab_rho_max=rmax,
+                        interp=interp, ew_alpha=alpha, tab_fp32=1)
+    assert rel_err(g, ref32).max() <= 1e-10
+    from paper_2602_20787_b200 import binding as b
+    g = gpu_accel_table(torch_cuda, (x, y, z, m, h), L, G, tab_nrho=nrho, tab_nz=nz, tab_rho_max=rmax,
+                        interp=interp, ew_alpha=alpha, precision=b.PREC_MIXED)
+    e = rel_err(g, ref32)
+    assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4
