@@ -171,3 +171,47 @@ def test_table_mode_randomised_parameters(torch_cuda, oracle, seed):
                         interp=interp, ew_alpha=alpha, precision=b.PREC_MIXED)
     e = rel_err(g, ref32)
     assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4
+
+
+def test_kdk_step_in_table_mode_is_the_same_leapfrog(torch_cuda, oracle):
+    """steps_cyl_kdk_step is mode-agnostic plumbing around the force call: in EWALD_TABLE mode one step must
+    equal the leapfrog of reading S4 written out here with the oracle's table-mode accelerations and its
+    Eq. 10 background (the kick / drift formulas themselves are pinned in test_oracle_background_kdk.py)."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(3, n=2500)
+    c = w.cosmo
+    nrho, nz, rmax = 48, 40, 400.0
+    D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, nrho, nz, rmax)
+    a0 = c["a_init"]
+    H0 = oracle.hubble(a0, c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+    a1, H1 = oracle.friedmann_rk4(a0, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+    dt = c["dt"]
+    # oracle side, step by step (reading S4): kick1 + drift, force, kick2
+    g0 = np.stack(oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, 0), 1)
+    bx, by = oracle.background(w.x, w.y, w.R_sim, 0.0, w.G, w.rho0, 1)
+    v = np.stack([w.vx, w.vy, w.vz], 1)
+    acc = g0.copy(); acc[:, 0] += bx; acc[:, 1] += by
+    v = v + 0.5 * dt * (acc / a0 ** 3 - 2.0 * H0 * v)
+    x, y = w.x + v[:, 0] * dt, w.y + v[:, 1] * dt
+    z = np.mod(w.z + v[:, 2] * dt, w.Lz)
+    g1 = np.stack(oracle.accel_table(x, y, z, w.m, w.h, w.Lz, w.G, D, rmax, 0), 1)
+    bx, by = oracle.background(x, y, w.R_sim, 0.0, w.G, w.rho0, 1)
+    acc = g1.copy(); acc[:, 0] += bx; acc[:, 1] += by
+    v = (v + 0.5 * dt * acc / a1 ** 3) / (1.0 + H1 * dt)
+    # GPU side
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, periodic_mode=b.PERIODIC_EWALD_TABLE, tab_nrho=nrho, tab_nz=nz,
+                     tab_rho_max=rmax, background=b.BG_INFINITE, R_sim=w.R_sim, rho0=w.rho0)
+    dev = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k))).cuda()
+           for k in ("x", "y", "z", "vx", "vy", "vz", "m", "h")}
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+    ctx.kdk_step(*[dev[k] for k in ("x", "y", "z", "vx", "vy", "vz", "m", "h")], *g, a0, H0, a1, H1, dt)
+    ctx.check()
+    ctx.close()
+    gv = np.stack([dev[k].cpu().numpy() for k in ("vx", "vy", "vz")], 1)
+    assert np.abs(dev["x"].cpu().numpy() - x).max() <= 1e-12 * np.abs(x).max()
+    assert np.abs(gv - v).max() <= 1e-10 * np.abs(v).max()
+    gg = np.stack([t.cpu().numpy() for t in g], 1)
+    assert (np.linalg.norm(gg - g1, axis=1) / np.linalg.norm(g1, axis=1)).max() <= 1e-10
