@@ -38,8 +38,11 @@ KERNEL_MIX = {
     # default fp64 kernel, pair_fp64_sym_kernel<5>: one unordered pair per iteration
     "fp64": dict(kernel="pair_fp64_sym_kernel<5>", interactions=2, dfma=53, dmul=33, dadd=22, dsetp=0,
                  per_image=(9.5, 14.0)),
-    # STEPS_FLAG_DETERMINISTIC, pair_fp64_kernel<5,0>: one ordered pair per iteration
-    "fp64_det": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
+    # STEPS_FLAG_DETERMINISTIC, pair_fp64_round_kernel<5>: the same loop, scheduled in conflict-free rounds
+    "fp64_det": dict(kernel="pair_fp64_round_kernel<5>", interactions=2, dfma=53, dmul=33, dadd=22, dsetp=0,
+                     per_image=(9.5, 14.0)),
+    # STEPS_FLAG_ORDERED_PAIRS, pair_fp64_kernel<5,0>: one ordered pair per iteration
+    "fp64_ord": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
                      per_image=(9.5, 14.0)),
     # --periodic table: pair_table_sym_kernel<CIC> (softened nearest image + 4 table gathers), one
     # unordered pair per iteration; independent of n_cut
@@ -252,6 +255,7 @@ def run_ours(args):
                      periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
                      tab_fp32=1 if (table and args.table_fp32) else 0,
                      flags=(b.FLAG_DETERMINISTIC if args.deterministic else 0)
+                     | (b.FLAG_ORDERED_PAIRS if args.ordered else 0)
                      | (b.FLAG_FAR_ORDER2 if args.far_order2 else 0))
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
@@ -313,6 +317,8 @@ def run_ours(args):
         mode = "mixed_table" if prec == b.PREC_MIXED else "table"
     else:
         mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
+        if args.ordered:
+            mode = "mixed_det" if prec == b.PREC_MIXED else "fp64_ord"
     instr, flops = pipe_counts(mode, args.n_cut)
     if args.far_order2 and mode == "fp64":              # one DFMA less per far image
         instr -= (2 * args.n_cut - 1) / 2.0
@@ -401,7 +407,9 @@ def main():
                     help="--periodic table: float table held in shared memory (tab_fp32 = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--deterministic", action="store_true",
-                    help="fp64: ordered-pair kernel with fixed-order reduction (STEPS_FLAG_DETERMINISTIC)")
+                    help="STEPS_FLAG_DETERMINISTIC: bit-reproducible (fp64: round-scheduled symmetric kernel)")
+    ap.add_argument("--ordered", action="store_true",
+                    help="STEPS_FLAG_ORDERED_PAIRS: ordered-pair kernels with fixed-order reduction")
     args = ap.parse_args()
     if args.warmup < 3:
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)

@@ -70,14 +70,19 @@ enum { STEPS_INTERP_CIC = 0,           /* cloud-in-cell: bilinear in (rho, z)   
 enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz                                    */
        STEPS_BG_INFINITE = 1           /* Eq. 10                                                       */ };
 
-enum { STEPS_FLAG_DETERMINISTIC = 1,   /* fp64 mode: evaluate every ORDERED pair and reduce in a fixed
-                                          order (bit-reproducible, ~1.9x slower) instead of the default
-                                          kernel, which evaluates every unordered pair once and applies
-                                          it to both particles with floating-point atomics (same terms,
-                                          summation order varies from run to run)                      */
-       STEPS_FLAG_FAR_ORDER2 = 2       /* fp64 images mode, default kernel only: the rsqrt refinement of
+enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default kernels evaluate every
+                                          unordered pair once and add it to both particles with
+                                          floating-point atomics (same terms, summation order varies from
+                                          run to run, ~1e-16).  With this flag the fp64 images mode
+                                          schedules the same evaluation in conflict-free rounds with
+                                          plain stores (~5 % slower); mixed precision falls back to an
+                                          ordered-pair kernel (~2.5x slower)                            */
+       STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,
-                                          per-particle error ~3e-12 instead of ~1e-14 (bar: 1e-10)     */ };
+                                          per-particle error ~3e-12 instead of ~1e-14 (bar: 1e-10)     */
+       STEPS_FLAG_ORDERED_PAIRS = 4    /* fp64 / mixed images mode: the literal form of Eq. 1 -- every target
+                                          sums over all its sources (ordered pairs, fixed-order reduction,
+                                          bit-reproducible, ~1.9x slower than the default)             */ };
 
 typedef struct steps_cyl_ctx steps_cyl_ctx;   /* opaque; created by init, freed by destroy */
 

@@ -18,6 +18,7 @@ PREC_FP64, PREC_MIXED = 0, 1
 BG_FINITE, BG_INFINITE = 0, 1
 FLAG_DETERMINISTIC = 1
 FLAG_FAR_ORDER2 = 2
+FLAG_ORDERED_PAIRS = 4
 INTERP_CIC, INTERP_TSC = 0, 1
 
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",

@@ -200,4 +200,115 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Deterministic variant (STEPS_FLAG_DETERMINISTIC): the same unordered-pair evaluation, scheduled in
+// ROUNDS so that no two CTAs ever update the same accumulator in one launch, and plain
+// read-modify-writes replace the atomics.  With T tiles (T even) and CTA b owning target tiles 2b and
+// 2b+1, round r gives CTA b the source tile t = (2b + r) mod T: distinct CTAs get distinct source
+// tiles, so the source-side sums acc_j[.][tile t] have one writer per round, and the target-side sums
+// acc_i[.][tiles 2b, 2b+1] only ever have their owner.  A tile pair (tt, t) with cyclic offset
+// o = (t - tt) mod T is taken when 0 < o < T/2, or o == T/2 and tt < t, or o == 0 (the tile against
+// itself, sub-tile rules as above); the other half of the offsets is the same pair seen from t.
+// Rounds r = 0 .. min(T/2 + 1, T - 1) are launched one after the other on the stream, so every
+// accumulator receives its contributions in a fixed order: bit-reproducible results at ~95 % of the
+// atomic kernel's speed (one tile of work per CTA per launch; T/2 + 2 launches per evaluation).
+// acc_i: [4][n_pad], acc_j: [3][n_pad], both zeroed by the host before round 0.
+template <int NC>
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
+pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                       const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                       int n_pad, int n_tiles, int round, int ncut_rt, PairConsts k,
+                       const DevFlags *__restrict__ flags, double *__restrict__ acc_i,
+                       double *__restrict__ acc_j)
+{
+    static_assert(SYM_R == 2, "round scheduling is written for two target tiles per CTA");
+    const int tb = blockIdx.x * SYM_R;
+    const int t = (tb + round) % n_tiles;
+    int mode[SYM_R];                                      // 0 skip, 1 both ways, 2 the tile against itself
+    {
+        const int half = n_tiles / 2;
+#pragma unroll
+        for (int r = 0; r < SYM_R; ++r) {
+            const int tt = tb + r, o = (t - tt + n_tiles) % n_tiles;
+            mode[r] = (o == 0) ? 2 : ((o < half || (o == half && tt < t)) ? 1 : 0);
+        }
+    }
+    if (mode[0] == 0 && mode[1] == 0) return;
+    {
+        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
+        if ((2.0 * hmax > k.halfL) || flags->bad_h) return;      // general kernel's job
+    }
+    __shared__ SymSrc s_src[PAIR_THREADS];
+    __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    SymTgt ti[SYM_R];
+    double a[SYM_R][4];
+    int soft_hi[SYM_R];
+    const double hm = tile_hmax[t];
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+        const double2 pi = xy[i], qi = zm[i];
+        ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
+        ti[r].mL = -k.L * qi.y;
+        a[r][0] = a[r][1] = a[r][2] = a[r][3] = 0.0;
+        const double b = ti[r].h + hm;
+        soft_hi[r] = hi32(b * b);
+    }
+    const int j = t * PAIR_THREADS + threadIdx.x;
+    {
+        const double2 pj = xy[j], qj = zm[j];
+        SymSrc v;
+        v.x = pj.x; v.y = pj.y; v.z = qj.x; v.m = qj.y; v.h = hs[j]; v.pad = 0.0;
+        s_src[threadIdx.x] = v;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+        double bx = 0.0, by = 0.0, bz = 0.0;
+        const SymSrc *sub = s_src + js * 32;
+        if (mode[0] == 1 && mode[1] == 1) {
+            ring_subtile<NC, SYM_R, true, false>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+        } else {
+#pragma unroll
+            for (int r = 0; r < SYM_R; ++r) {
+                if (mode[r] == 0) continue;
+                const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
+                const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
+                double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
+                double cx = 0.0, cy = 0.0, cz = 0.0;
+                if (mode[r] == 1 || js > w)
+                    ring_subtile<NC, 1, true, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                else if (js == w)
+                    ring_subtile<NC, 1, false, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                bx += cx; by += cy; bz += cz;
+            }
+        }
+        const int jl = js * 32 + lane;
+        s_b[w][0][jl] = bx;
+        s_b[w][1][jl] = by;
+        s_b[w][2][jl] = bz;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double v = s_b[0][c][threadIdx.x];
+#pragma unroll
+        for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
+        double *p = acc_j + (size_t)c * n_pad + j;            // this CTA is the tile's only writer this round
+        *p = *p - v;
+    }
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        if (mode[r] == 0) continue;
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            double *p = acc_i + (size_t)c * n_pad + i;        // only the owner CTA ever writes these
+            *p = *p + a[r][c];
+        }
+    }
+}
+
 }  // namespace steps

@@ -28,6 +28,7 @@ struct steps_cyl_ctx {
     int n_chunks, tiles_per_chunk;
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
     bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
+    bool use_rounds;                              // fp64 + DETERMINISTIC: round-scheduled symmetric kernel
     int sm_count;
     PairConsts kc;
     MixedConsts mc;
@@ -142,6 +143,19 @@ void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
                                                                      c->kc, c->flags, c->part);
 }
 
+// Deterministic fp64 path: rounds of the symmetric evaluation, one launch each (pair_fp64_sym.cuh).
+template <int NC>
+void launch_pair_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
+    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad;
+    for (int r = 0; r <= last; ++r)
+        pair_fp64_round_kernel<NC><<<T / SYM_R, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+                                                                    c->n_pad, T, r, c->p.n_cut, c->kc,
+                                                                    c->flags, acc_i, acc_j);
+    c->launches += last;      // launch_pair() adds the remaining 2
+}
+
 template <int NC>
 void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
@@ -205,6 +219,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<N>(c, s); \
         else if (mixed) launch_pair_mixed_nc<N>(c, s);           \
         else if (c->use_sym) launch_pair_sym_nc<N>(c, s);        \
+        else if (c->use_rounds) launch_pair_rounds_nc<N>(c, s);  \
         else launch_pair_fp64_nc<N>(c, s);                       \
         break;
         CASE_NC(1) CASE_NC(2) CASE_NC(3) CASE_NC(4) CASE_NC(5) CASE_NC(6) CASE_NC(7) CASE_NC(8)
@@ -213,6 +228,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<0>(c, s);
         else if (mixed) launch_pair_mixed_nc<0>(c, s);
         else if (c->use_sym) launch_pair_sym_nc<0>(c, s);
+        else if (c->use_rounds) launch_pair_rounds_nc<0>(c, s);
         else launch_pair_fp64_nc<0>(c, s);
     }
     // general path: a no-op unless 2 max(h) > L/2
@@ -234,13 +250,15 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
                                                      ctx->tile_hmax, ctx->flags);
     ctx->launches += 1;
     CK(cudaEventRecord(ctx->ev0, s));
-    if (ctx->use_sym)      // the symmetric kernel accumulates with atomics into part[0..4 n_pad)
+    if (ctx->use_sym)      // the symmetric kernels accumulate with atomics into part[0..4 n_pad)
         CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * sizeof(double), s));
+    if (ctx->use_rounds)   // target-side sums in slab 0, source-side sums in slab 1 (its 4th row stays 0)
+        CK(cudaMemsetAsync(ctx->part, 0, 8 * (size_t)ctx->n_pad * sizeof(double), s));
     launch_pair(ctx, s);
     CK(cudaEventRecord(ctx->ev1, s));
     ctx->ev_valid = true;
     finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
-                                                         ctx->use_sym ? 1 : ctx->n_chunks,
+                                                         ctx->use_sym ? 1 : (ctx->use_rounds ? 2 : ctx->n_chunks),
                                                          ctx->table_mode ? 1 : ctx->n_chunks,
                                                          ctx->kc.halfL, ctx->flags,
                                                          ctx->p.G, ctx->p.Lz, gx, gy, gz);
@@ -276,7 +294,9 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         return STEPS_EINVAL;
     if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
     if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
-    if ((p->flags & ~(STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_FAR_ORDER2)) != 0 || p->device < 0) return STEPS_EINVAL;
+    if ((p->flags & ~(STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_FAR_ORDER2 | STEPS_FLAG_ORDERED_PAIRS)) != 0 ||
+        p->device < 0)
+        return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
     if (p->rho0 != 0.0 && p->background == STEPS_BG_FINITE && !(p->R_sim > 0.0)) return STEPS_EINVAL;
     if (p->tab_fp32 != 0 && p->tab_fp32 != 1) return STEPS_EINVAL;
@@ -293,7 +313,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             !(pp.tab_rho_max > 0.0) || !std::isfinite(pp.tab_rho_max) ||
             (pp.interp != STEPS_INTERP_CIC && pp.interp != STEPS_INTERP_TSC))
             return STEPS_EINVAL;
-        if (p->flags & STEPS_FLAG_DETERMINISTIC) return STEPS_EUNSUPPORTED;
+        if (p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS)) return STEPS_EUNSUPPORTED;
         if (p->precision == STEPS_PREC_MIXED) pp.tab_fp32 = 1;      // mixed mode always uses the float table
     }
 
@@ -319,7 +339,9 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     }
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
-    ctx->use_sym = !(p->flags & STEPS_FLAG_DETERMINISTIC);
+    ctx->use_sym = !(p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS));
+    ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS) &&
+                      p->precision == STEPS_PREC_FP64 && p->periodic_mode == STEPS_PERIODIC_IMAGES;
 
     const double L = p->Lz;
     ctx->kc.L = L;
@@ -352,7 +374,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->tile_hmax, (size_t)ctx->n_tiles));
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
-    A(dev_alloc(&ctx->part, np * 4 * (size_t)ctx->n_chunks));
+    A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 2)));
     A(dev_alloc(&ctx->bx, np));
     A(dev_alloc(&ctx->by, np));
     A(dev_alloc(&ctx->flags, 1));

@@ -45,7 +45,8 @@ def main():
         ref = np.stack(oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, w.n_cut, targets=idx), 1)
         dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.x, w.y, w.z, w.m, w.h)]
         for name, prec, flags in (("fp64 (symmetric, default)", b.PREC_FP64, 0),
-                                  ("fp64 deterministic", b.PREC_FP64, b.FLAG_DETERMINISTIC),
+                                  ("fp64 deterministic (rounds)", b.PREC_FP64, b.FLAG_DETERMINISTIC),
+                                  ("fp64 ordered pairs", b.PREC_FP64, b.FLAG_ORDERED_PAIRS),
                                   ("mixed", b.PREC_MIXED, 0)):
             ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=w.n_cut, precision=prec, flags=flags)
             g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]

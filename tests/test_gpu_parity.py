@@ -202,17 +202,19 @@ def test_bench_size_sampled_targets(torch_cuda, oracle, precision):
         assert abs(np.sum(w.m * c)) <= (1e-11 if precision == 0 else 1e-5) * np.sum(w.m * np.abs(c))
 
 
-@pytest.mark.parametrize("n", [2, 129, 700, 5000])
-def test_deterministic_ordered_kernel(torch_cuda, oracle, n):
-    """STEPS_FLAG_DETERMINISTIC: the ordered-pair kernel with fixed-order reduction -- same parity
-    bar, and bit-identical results from run to run."""
+@pytest.mark.parametrize("n", [2, 129, 257, 700, 5000])
+@pytest.mark.parametrize("flag", [1, 4])
+def test_deterministic_kernels(torch_cuda, oracle, n, flag):
+    """STEPS_FLAG_DETERMINISTIC (round-scheduled symmetric kernel, plain stores) and
+    STEPS_FLAG_ORDERED_PAIRS (ordered pairs, fixed-order reduction): same parity bar, and bit-identical
+    results from run to run."""
     from paper_2602_20787_b200 import binding as b
     from paper_2602_20787_b200 import workloads
     w = workloads.make(1, n=n, seed=21)
     arrs = (w.x, w.y, w.z, w.m, w.h)
     ref = oracle.accel(*arrs, w.Lz, w.G, 5)
-    g1 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_DETERMINISTIC)
-    g2 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=b.FLAG_DETERMINISTIC)
+    g1 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=flag)
+    g2 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 0, flags=flag)
     check(g1, ref, 0)
     for a, c in zip(g1, g2):
         assert np.array_equal(a, c)
@@ -276,5 +278,6 @@ def test_randomised_parameters(torch_cuda, oracle, seed):
     for precision in (0, 1):
         g = gpu_accel(torch_cuda, (x, y, z, m, h), L, G, n_cut, precision)
         check(g, ref, 0 if general else precision)
-    g = gpu_accel(torch_cuda, (x, y, z, m, h), L, G, n_cut, 0, flags=1)
-    check(g, ref, 0)
+    for flag in (1, 4):
+        g = gpu_accel(torch_cuda, (x, y, z, m, h), L, G, n_cut, 0, flags=flag)
+        check(g, ref, 0)
