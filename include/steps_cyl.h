@@ -75,7 +75,7 @@ enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default
                                           floating-point atomics (same terms, summation order varies from
                                           run to run, ~1e-16).  With this flag the fp64 images mode
                                           schedules the same evaluation in conflict-free rounds with
-                                          plain stores (~5 % slower); mixed precision falls back to an
+                                          plain stores (~3 % slower); mixed precision falls back to an
                                           ordered-pair kernel (~2.5x slower)                            */
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,

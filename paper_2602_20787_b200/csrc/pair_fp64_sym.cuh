@@ -25,7 +25,7 @@
 //
 // Results are accumulated with floating-point atomics, so the summation ORDER (not the set of
 // terms) can differ from run to run: results are reproducible to round-off (~1e-16 relative),
-// not bit for bit.  STEPS_FLAG_DETERMINISTIC selects pair_fp64_kernel instead.
+// not bit for bit.  STEPS_FLAG_DETERMINISTIC selects pair_fp64_round_kernel (end of this file).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -210,7 +210,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
 // o = (t - tt) mod T is taken when 0 < o < T/2, or o == T/2 and tt < t, or o == 0 (the tile against
 // itself, sub-tile rules as above); the other half of the offsets is the same pair seen from t.
 // Rounds r = 0 .. min(T/2 + 1, T - 1) are launched one after the other on the stream, so every
-// accumulator receives its contributions in a fixed order: bit-reproducible results at ~95 % of the
+// accumulator receives its contributions in a fixed order: bit-reproducible results at ~97 % of the
 // atomic kernel's speed (one tile of work per CTA per launch; T/2 + 2 launches per evaluation).
 // acc_i: [4][n_pad], acc_j: [3][n_pad], both zeroed by the host before round 0.
 template <int NC>
