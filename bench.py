@@ -57,8 +57,11 @@ KERNEL_MIX = {
     # here as scalar FP32 operations per unordered pair)
     "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=38, fmul=19, fadd=16, mufu=10,
                   f2f=0, dadd=0),
-    # STEPS_FLAG_DETERMINISTIC, pair_mixed_kernel<5>: one ordered pair per iteration
-    "mixed_det": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
+    # STEPS_FLAG_DETERMINISTIC, pair_mixed_round_kernel<5>: the same loop in conflict-free rounds
+    "mixed_det": dict(kernel="pair_mixed_round_kernel<5>", interactions=2, ffma=38, fmul=19, fadd=16, mufu=10,
+                      f2f=0, dadd=0),
+    # STEPS_FLAG_ORDERED_PAIRS, pair_mixed_kernel<5>: one ordered pair per iteration
+    "mixed_ord": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
                       f2f=4, dadd=4),
 }
 METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
@@ -318,7 +321,7 @@ def run_ours(args):
     else:
         mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
         if args.ordered:
-            mode = "mixed_det" if prec == b.PREC_MIXED else "fp64_ord"
+            mode = "mixed_ord" if prec == b.PREC_MIXED else "fp64_ord"
     instr, flops = pipe_counts(mode, args.n_cut)
     if args.far_order2 and mode == "fp64":              # one DFMA less per far image
         instr -= (2 * args.n_cut - 1) / 2.0

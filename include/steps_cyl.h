@@ -73,10 +73,9 @@ enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz             
 enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default kernels evaluate every
                                           unordered pair once and add it to both particles with
                                           floating-point atomics (same terms, summation order varies from
-                                          run to run, ~1e-16).  With this flag the fp64 images mode
+                                          run to run, ~1e-16).  With this flag the images mode
                                           schedules the same evaluation in conflict-free rounds with
-                                          plain stores (~3 % slower); mixed precision falls back to an
-                                          ordered-pair kernel (~2.5x slower)                            */
+                                          plain stores (~3 % slower)                                    */
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,
                                           per-particle error ~3e-12 instead of ~1e-14 (bar: 1e-10)     */

@@ -352,4 +352,117 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
     }
 }
 
+// Deterministic variant in rounds: the scheduling of pair_fp64_round_kernel (pair_fp64_sym.cuh) with the
+// float pair arithmetic of this file.  acc_i: [4][n_pad], acc_j: [3][n_pad], zeroed before round 0.
+template <int NC>
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
+pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
+                        const double *__restrict__ tile_hmax, int n_pad, int n_tiles, int round,
+                        int ncut_rt, MixedConsts k, double halfL, const DevFlags *__restrict__ flags,
+                        double *__restrict__ acc_i, double *__restrict__ acc_j)
+{
+    static_assert(SYM_R == 2, "round scheduling is written for two target tiles per CTA");
+    const int tb = blockIdx.x * SYM_R;
+    const int t = (tb + round) % n_tiles;
+    int mode[SYM_R];                                      // 0 skip, 1 both ways, 2 the tile against itself
+    {
+        const int half = n_tiles / 2;
+#pragma unroll
+        for (int r = 0; r < SYM_R; ++r) {
+            const int tt = tb + r, o = (t - tt + n_tiles) % n_tiles;
+            mode[r] = (o == 0) ? 2 : ((o < half || (o == half && tt < t)) ? 1 : 0);
+        }
+    }
+    if (mode[0] == 0 && mode[1] == 0) return;
+    {
+        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
+        if ((2.0 * hmax > halfL) || flags->bad_h) return;
+    }
+    __shared__ float4 s_hi[PAIR_THREADS];
+    __shared__ float4 s_lo[PAIR_THREADS];
+    __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    MixTgt ti[SYM_R];
+    double A[SYM_R][4];
+    int soft_bits[SYM_R];
+    const float hm = (float)tile_hmax[t] * 1.0001f;
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+        const float4 h4 = f_hi[i], l4 = f_lo[i];
+        ti[r].xh = h4.x; ti[r].yh = h4.y; ti[r].zh = h4.z; ti[r].m = h4.w;
+        ti[r].xl = l4.x; ti[r].yl = l4.y; ti[r].zl = l4.z; ti[r].h = l4.w;
+        ti[r].mL = -k.Lh * h4.w;
+        A[r][0] = A[r][1] = A[r][2] = A[r][3] = 0.0;
+        const float b = (ti[r].h + hm) * 1.0001f;
+        soft_bits[r] = __float_as_int(b * b);
+    }
+    MixTgt2 ti2;
+    ti2.xh = make_float2(ti[0].xh, ti[1].xh); ti2.yh = make_float2(ti[0].yh, ti[1].yh);
+    ti2.zh = make_float2(ti[0].zh, ti[1].zh); ti2.xl = make_float2(ti[0].xl, ti[1].xl);
+    ti2.yl = make_float2(ti[0].yl, ti[1].yl); ti2.zl = make_float2(ti[0].zl, ti[1].zl);
+    ti2.h = make_float2(ti[0].h, ti[1].h);    ti2.m = make_float2(ti[0].m, ti[1].m);
+    ti2.mL = make_float2(ti[0].mL, ti[1].mL);
+    const int j = t * PAIR_THREADS + threadIdx.x;
+    s_hi[threadIdx.x] = f_hi[j];
+    s_lo[threadIdx.x] = f_lo[j];
+    __syncthreads();
+#pragma unroll 1
+    for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+        float bx = 0.0f, by = 0.0f, bz = 0.0f;
+        const float4 *sh = s_hi + js * 32, *sl = s_lo + js * 32;
+        if (mode[0] == 1 && mode[1] == 1) {
+            float2 a2[4], b2x, b2y, b2z;
+            ring_subtile_f32x2<NC>(ti2, soft_bits, sh, sl, lane, k, ncut_rt, a2, b2x, b2y, b2z);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                A[0][c] += (double)a2[c].x;
+                A[1][c] += (double)a2[c].y;
+            }
+            bx = b2x.x + b2x.y;
+            by = b2y.x + b2y.y;
+            bz = b2z.x + b2z.y;
+        } else {
+#pragma unroll
+            for (int r = 0; r < SYM_R; ++r) {
+                if (mode[r] == 0) continue;
+                const MixTgt (&t1r)[1] = reinterpret_cast<const MixTgt (&)[1]>(ti[r]);
+                const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_bits[r]);
+                float a1[1][4] = {{0.0f, 0.0f, 0.0f, 0.0f}};
+                float cx = 0.0f, cy = 0.0f, cz = 0.0f;
+                if (mode[r] == 1 || js > w)
+                    ring_subtile_f32<NC, 1, true>(t1r, s1r, sh, sl, lane, k, ncut_rt, a1, cx, cy, cz);
+                else if (js == w)
+                    ring_subtile_f32<NC, 1, false>(t1r, s1r, sh, sl, lane, k, ncut_rt, a1, cx, cy, cz);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) A[r][c] += (double)a1[0][c];
+                bx += cx; by += cy; bz += cz;
+            }
+        }
+        const int jl = js * 32 + lane;
+        s_b[w][0][jl] = bx;
+        s_b[w][1][jl] = by;
+        s_b[w][2][jl] = bz;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double v = (double)s_b[0][c][threadIdx.x];
+#pragma unroll
+        for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += (double)s_b[ww][c][threadIdx.x];
+        double *p = acc_j + (size_t)c * n_pad + j;
+        *p = *p - v;
+    }
+#pragma unroll
+    for (int r = 0; r < SYM_R; ++r) {
+        if (mode[r] == 0) continue;
+        const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            double *p = acc_i + (size_t)c * n_pad + i;
+            *p = *p + A[r][c];
+        }
+    }
+}
+
 }  // namespace steps

@@ -28,7 +28,7 @@ struct steps_cyl_ctx {
     int n_chunks, tiles_per_chunk;
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
     bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
-    bool use_rounds;                              // fp64 + DETERMINISTIC: round-scheduled symmetric kernel
+    bool use_rounds;                              // DETERMINISTIC: round-scheduled symmetric kernels
     int sm_count;
     PairConsts kc;
     MixedConsts mc;
@@ -157,6 +157,18 @@ void launch_pair_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
 }
 
 template <int NC>
+void launch_pair_mixed_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
+{
+    const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
+    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad;
+    for (int r = 0; r <= last; ++r)
+        pair_mixed_round_kernel<NC><<<T / SYM_R, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax,
+                                                                     c->n_pad, T, r, c->p.n_cut, c->mc,
+                                                                     c->kc.halfL, c->flags, acc_i, acc_j);
+    c->launches += last;
+}
+
+template <int NC>
 void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles, c->n_chunks);
@@ -217,6 +229,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 #define CASE_NC(N)                                               \
     case N:                                                      \
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<N>(c, s); \
+        else if (mixed && c->use_rounds) launch_pair_mixed_rounds_nc<N>(c, s); \
         else if (mixed) launch_pair_mixed_nc<N>(c, s);           \
         else if (c->use_sym) launch_pair_sym_nc<N>(c, s);        \
         else if (c->use_rounds) launch_pair_rounds_nc<N>(c, s);  \
@@ -226,6 +239,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 #undef CASE_NC
     default:
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<0>(c, s);
+        else if (mixed && c->use_rounds) launch_pair_mixed_rounds_nc<0>(c, s);
         else if (mixed) launch_pair_mixed_nc<0>(c, s);
         else if (c->use_sym) launch_pair_sym_nc<0>(c, s);
         else if (c->use_rounds) launch_pair_rounds_nc<0>(c, s);
@@ -341,7 +355,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     choose_chunks(ctx);
     ctx->use_sym = !(p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS));
     ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS) &&
-                      p->precision == STEPS_PREC_FP64 && p->periodic_mode == STEPS_PERIODIC_IMAGES;
+                      p->periodic_mode == STEPS_PERIODIC_IMAGES;
 
     const double L = p->Lz;
     ctx->kc.L = L;

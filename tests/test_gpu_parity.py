@@ -223,16 +223,18 @@ def test_deterministic_kernels(torch_cuda, oracle, n, flag):
     assert rel_err(g3, g1).max() < 1e-12
 
 
-def test_deterministic_mixed_kernel(torch_cuda, oracle):
-    """Mixed precision with STEPS_FLAG_DETERMINISTIC: ordered-pair kernel, each pair contribution
-    converted to double before it is added; bit-identical from run to run."""
+@pytest.mark.parametrize("flag", [1, 4])
+def test_deterministic_mixed_kernel(torch_cuda, oracle, flag):
+    """Mixed precision with STEPS_FLAG_DETERMINISTIC (round-scheduled symmetric kernel) or
+    STEPS_FLAG_ORDERED_PAIRS (ordered pairs, each contribution converted to double before it is
+    added): bit-identical from run to run."""
     from paper_2602_20787_b200 import binding as b
     from paper_2602_20787_b200 import workloads
     w = workloads.make(1, n=3000, seed=23)
     arrs = (w.x, w.y, w.z, w.m, w.h)
     ref = oracle.accel(*arrs, w.Lz, w.G, 5)
-    g1 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 1, flags=b.FLAG_DETERMINISTIC)
-    g2 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 1, flags=b.FLAG_DETERMINISTIC)
+    g1 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 1, flags=flag)
+    g2 = gpu_accel(torch_cuda, arrs, w.Lz, w.G, 5, 1, flags=flag)
     check(g1, ref, 1)
     for a, c in zip(g1, g2):
         assert np.array_equal(a, c)
