@@ -17,3 +17,10 @@ def oracle():
     import oracle as _o
     _o.build()
     return _o
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """Compile libsteps_cyl.so if it is missing or stale (content hash); a no-op otherwise."""
+    from paper_2602_20787_b200 import build
+    build.build()
