@@ -1,5 +1,5 @@
 #!/usr/bin/env python
-"""Full-size parity report: BASELINE.json configs 1-4 at their full particle counts, GPU (through
+"""Full-size parity report: BASELINE.json configs 0-4 at their full particle counts, GPU (through
 the C ABI) against the CPU oracle on seeded sampled targets x all sources, both precisions.
 
     python tests/fullsize_parity.py [--configs 1,2,3,4] [--targets 256] > gpurun_out/fullsize.md
@@ -20,7 +20,7 @@ sys.path.insert(0, ROOT)
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="1,2,3,4")
+    ap.add_argument("--configs", default="0,1,2,3,4")
     ap.add_argument("--targets", type=int, default=256)
     ap.add_argument("--n", type=int, default=0, help="override N (debugging)")
     args = ap.parse_args()
@@ -57,7 +57,7 @@ def main():
             ctx.close()
             e = np.linalg.norm(got[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
             mom = max(abs(np.sum(w.m * got[:, c])) / np.sum(w.m * np.abs(got[:, c])) for c in range(3))
-            print("| %d | %d | %s | %d | %.2e | %.2e | %.3f | %.1e |"
+            print("| %d | %d | %s | %d | %.2e | %.2e | %.4g | %.1e |"
                   % (cfg, w.n, name, len(idx), e.max(), np.sqrt(np.mean(e ** 2)), secs, mom), flush=True)
 
 
