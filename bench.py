@@ -257,6 +257,7 @@ def run_ours(args):
                      R_sim=w.R_sim, rho0=w.rho0, device=local,
                      periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
                      tab_fp32=1 if (table and args.table_fp32) else 0,
+                     interp=b.INTERP_TSC if (table and args.interp == "tsc") else b.INTERP_CIC,
                      flags=(b.FLAG_DETERMINISTIC if args.deterministic else 0)
                      | (b.FLAG_ORDERED_PAIRS if args.ordered else 0)
                      | (b.FLAG_FAR_ORDER2 if args.far_order2 else 0))
@@ -365,8 +366,8 @@ def run_ours(args):
         cpu = {"value": len(idx) * (n - 1) / tc, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
                          "%.1f s" % (len(idx), n, tc)}
-    periodic_desc = ("Ewald table 144x128 CIC%s, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10"
-                     % (" (float nodes in shared memory)" if (args.table_fp32 or prec == b.PREC_MIXED) else "") if table
+    periodic_desc = ("Ewald table 144x128 %s%s, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10"
+                     % (args.interp.upper(), " (float nodes in shared memory)" if (args.table_fp32 or prec == b.PREC_MIXED) else "") if table
                      else "n_cut=%d (%d images/pair), background Eq. 9" % (args.n_cut, 2 * args.n_cut))
     line = {
         "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
@@ -406,6 +407,8 @@ def main():
                     help="CPU seconds of oracle work per sample / reference step")
     ap.add_argument("--far-order2", action="store_true",
                     help="fp64 images mode: STEPS_FLAG_FAR_ORDER2 (far images refined to first order only)")
+    ap.add_argument("--interp", default="cic", choices=["cic", "tsc"],
+                    help="--periodic table: cloud-in-cell (4 nodes) or triangular-shaped cloud (9 nodes)")
     ap.add_argument("--table-fp32", action="store_true",
                     help="--periodic table: float table held in shared memory (tab_fp32 = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

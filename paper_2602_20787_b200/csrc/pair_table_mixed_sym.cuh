@@ -15,26 +15,44 @@ struct TableConstsF32 {
     float rho_max2, inv_drho, inv_dz, two_over_L;
 };
 
+// floor(x) and frac(x) of 0 <= x < 2^22 without the quarter-rate conversion instructions.
+__device__ __forceinline__ void floor_frac_f32(float x, int &i, float &f)
+{
+    const float t = __fadd_rd(x, 8388608.0f);               // 2^23 + floor(x), exact
+    i = __float_as_int(t) - 0x4b000000;
+    f = x - (t - 8388608.0f);
+}
+
 // Interpolated {D_rho, D_z} in float; nodes from the shared-memory float2 table.
 template <int INTERP>
 __device__ __forceinline__ float2 table_lookup_f32(const TableConstsF32 &tc, const float2 *tab, float rho,
                                                   float az)
 {
     const float xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
+    const int nzs = tc.nz + 2;
     if (INTERP == 0) {
-        int i0 = __float2int_rd(xr), j0 = __float2int_rd(xz);
-        const float fr = xr - (float)i0, fz = xz - (float)j0;
-        const int i1 = min(i0 + 1, tc.nrho - 1), j1 = min(j0 + 1, tc.nz - 1);
-        i0 = min(i0, tc.nrho - 1);
-        j0 = min(j0, tc.nz - 1);
-        const float2 d00 = tab[i0 * tc.nz + j0], d01 = tab[i0 * tc.nz + j1];
-        const float2 d10 = tab[i1 * tc.nz + j0], d11 = tab[i1 * tc.nz + j1];
+        int i0, j0;
+        float fr, fz;
+        floor_frac_f32(xr, i0, fr);
+        floor_frac_f32(xz, j0, fz);
+        // lanes beyond rho_max (and the padding particles) arrive here too: any node will do for them
+        i0 = min(max(i0, 0), tc.nrho - 1);
+        j0 = min(max(j0, 0), tc.nz - 1);
+        const float2 *d = tab + (i0 + 1) * nzs + j0 + 1;    // haloed table: stage_table_halo()
+        const float2 d00 = d[0], d01 = d[1], d10 = d[nzs], d11 = d[nzs + 1];
         const float ax = fmaf(fz, d01.x - d00.x, d00.x), bx = fmaf(fz, d11.x - d10.x, d10.x);
         const float ay = fmaf(fz, d01.y - d00.y, d00.y), by = fmaf(fz, d11.y - d10.y, d10.y);
         return make_float2(fmaf(fr, bx - ax, ax), fmaf(fr, by - ay, ay));
     }
-    const int ic = __float2int_rd(xr + 0.5f), jc = __float2int_rd(xz + 0.5f);
-    const float dr = xr - (float)ic, dz = xz - (float)jc;
+    int ic, jc;
+    float dr, dz;
+    floor_frac_f32(xr + 0.5f, ic, dr);
+    floor_frac_f32(xz + 0.5f, jc, dz);
+    dr -= 0.5f;
+    dz -= 0.5f;
+    ic = min(max(ic, 0), tc.nrho - 1);
+    jc = min(max(jc, 0), tc.nz - 1);
+    const float2 *d = tab + ic * nzs + jc;                  // node (ic - 1, jc - 1)
     const float wr[3] = {0.5f * (0.5f - dr) * (0.5f - dr), 0.75f - dr * dr, 0.5f * (0.5f + dr) * (0.5f + dr)};
     const float wz[3] = {0.5f * (0.5f - dz) * (0.5f - dz), 0.75f - dz * dz, 0.5f * (0.5f + dz) * (0.5f + dz)};
     float ox = 0.0f, oy = 0.0f;
@@ -43,15 +61,9 @@ __device__ __forceinline__ float2 table_lookup_f32(const TableConstsF32 &tc, con
         float rx = 0.0f, ry = 0.0f;
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            int i = ic - 1 + a, j = jc - 1 + b;
-            float sr = 1.0f, sz = 1.0f;                     // boundary rules of reading T3
-            if (i < 0) { i = -i; sr = -1.0f; }
-            if (i > tc.nrho - 1) i = tc.nrho - 1;
-            if (j < 0) { j = -j; sz = -1.0f; }
-            if (j > tc.nz - 1) { j = 2 * (tc.nz - 1) - j; sz = -sz; }
-            const float2 v = tab[i * tc.nz + j];
-            rx = fmaf(wz[b], sr * v.x, rx);
-            ry = fmaf(wz[b], sz * v.y, ry);
+            const float2 v = d[a * nzs + b];
+            rx = fmaf(wz[b], v.x, rx);
+            ry = fmaf(wz[b], v.y, ry);
         }
         ox = fmaf(wr[a], rx, ox);
         oy = fmaf(wr[a], ry, oy);
@@ -73,36 +85,40 @@ __device__ __forceinline__ void ring_subtile_table_f32(const MixTgt (&ti)[R], co
     for (int s = 0; s < 32; ++s) {
         const int jj = (lane + s) & 31;
         const float4 jh = s_hi[jj], jl = s_lo[jj];
+        // three phases per source, as in ring_subtile_table (pair_table_sym.cuh): branch-free geometry +
+        // lookup for all R targets, then the rare spline correction, then selects and accumulation
+        float rx[R], ry[R], rz[R], q[R], w0[R], y[R];
+        float2 Dv[R];
+        bool near[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float rx = (ti[r].xh - jh.x) + (ti[r].xl - jl.x);
-            const float ry = (ti[r].yh - jh.y) + (ti[r].yl - jl.y);
-            float rz = (ti[r].zh - jh.z) + (ti[r].zl - jl.z);
-            if (fabsf(rz) > k.halfL) {                       // exact nearest image: |rz| <= L/2 afterwards
-                const float sg = copysignf(1.0f, rz);
-                rz = fmaf(-sg, k.Ll, fmaf(-sg, k.Lh, rz));
+            rx[r] = (ti[r].xh - jh.x) + (ti[r].xl - jl.x);
+            ry[r] = (ti[r].yh - jh.y) + (ti[r].yl - jl.y);
+            const float rz0 = (ti[r].zh - jh.z) + (ti[r].zl - jl.z);
+            // exact nearest image: |rz| <= L/2 afterwards
+            const float sg = (fabsf(rz0) > k.halfL) ? copysignf(1.0f, rz0) : 0.0f;
+            rz[r] = fmaf(-sg, k.Ll, fmaf(-sg, k.Lh, rz0));
+            const float rho2 = fmaf(ry[r], ry[r], rx[r] * rx[r]);
+            y[r] = (rho2 > 0.0f) ? rsqrt_f32(rho2) : 0.0f;
+            near[r] = rho2 < tc.rho_max2;
+            q[r] = fmaf(rz[r], rz[r], rho2);
+            w0[r] = inv_cube_sqrt_f32(q[r]);
+            Dv[r] = table_lookup_f32<INTERP>(tc, tab, rho2 * y[r], fabsf(rz[r]));
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (__float_as_int(q[r]) <= soft_bits[r]) {
+                const float hh = ti[r].h + jl.w;
+                if (q[r] < hh * hh) w0[r] = spline_w_f32(q[r], hh);
             }
-            const float rho2 = fmaf(ry, ry, rx * rx);
-            const float y = (rho2 > 0.0f) ? rsqrt_f32(rho2) : 0.0f;
-            float px, py, pz;
-            if (rho2 < tc.rho_max2) {
-                const float q = fmaf(rz, rz, rho2);
-                float w0 = inv_cube_sqrt_f32(q);
-                if (__float_as_int(q) <= soft_bits[r]) {
-                    const float hh = ti[r].h + jl.w;
-                    if (q < hh * hh) w0 = spline_w_f32(q, hh);
-                }
-                const float2 Dv = table_lookup_f32<INTERP>(tc, tab, rho2 * y, fabsf(rz));
-                const float cr = fmaf(-Dv.x, y, w0);
-                px = cr * rx;
-                py = cr * ry;
-                pz = fmaf(w0, rz, (rz < 0.0f) ? Dv.y : -Dv.y);
-            } else {
-                const float cr = tc.two_over_L * y * y;
-                px = cr * rx;
-                py = cr * ry;
-                pz = 0.0f;
-            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float cn = fmaf(-Dv[r].x, y[r], w0[r]);
+            const float cf = tc.two_over_L * y[r] * y[r];
+            const float zn = fmaf(w0[r], rz[r], (rz[r] < 0.0f) ? Dv[r].y : -Dv[r].y);
+            const float cr = near[r] ? cn : cf;
+            const float px = cr * rx[r], py = cr * ry[r], pz = near[r] ? zn : 0.0f;
             a[r][0] = fmaf(jh.w, px, a[r][0]);
             a[r][1] = fmaf(jh.w, py, a[r][1]);
             a[r][2] = fmaf(jh.w, pz, a[r][2]);
@@ -123,7 +139,7 @@ __device__ __forceinline__ void ring_subtile_table_f32(const MixTgt (&ti)[R], co
 
 constexpr int TABLE_MIXED_WARPS = 16;
 
-// grid = (n_tiles / 8, chunks), 512 threads; dynamic shared memory = 16*3*128 floats + nodes*8 bytes.
+// grid = (n_tiles / 8, chunks), 512 threads; dynamic shared memory = 16*3*128 floats + (nrho+2)(nz+2)*8 bytes.
 template <int INTERP>
 __global__ void __launch_bounds__(TABLE_MIXED_WARPS * 32, 1)
 pair_table_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
@@ -141,10 +157,7 @@ pair_table_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__res
     extern __shared__ float s_dynf[];
     float (*s_b)[3][PAIR_THREADS] = reinterpret_cast<float (*)[3][PAIR_THREADS]>(s_dynf);
     float2 *s_table = reinterpret_cast<float2 *>(s_dynf + TW * 3 * PAIR_THREADS);
-    {
-        const int nodes = tc.nrho * tc.nz;
-        for (int q = threadIdx.x; q < nodes; q += TW * 32) s_table[q] = table_f32[q];
-    }
+    stage_table_halo(s_table, table_f32, tc.nrho, tc.nz, TW * 32);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, wq = w & 3;
     const int tgt0 = tb + (w >> 2) * SYM_R;
     MixTgt ti[SYM_R];

@@ -46,17 +46,32 @@ __device__ __forceinline__ double rsqrt_full(double x)
 
 // Where the nodes live: double2 in global memory (read through L1), or float2 in shared memory.
 struct GlobalTable {
+    static constexpr bool kLookupAlways = false;   // gathers from L1: only lanes that need the node
     const double2 *D;
     __device__ __forceinline__ double2 node(int idx) const { return __ldg(D + idx); }
 };
 struct SharedTableF32 {
+    static constexpr bool kLookupAlways = true;    // shared memory: cheaper than a divergent branch
     const float2 *D;
-    __device__ __forceinline__ double2 node(int idx) const
-    {
-        const float2 v = D[idx];
-        return make_double2((double)v.x, (double)v.y);
-    }
 };
+
+// floor(x) and 1 + frac(x) (truncated to float) of 0 <= x < 2^31 from three FP64 additions and two
+// integer instructions: the conversion instructions (F2I.F64, I2F.F64, F2F) issue at a quarter of
+// the FP64 rate and were what bounded this kernel.
+__device__ __forceinline__ void floor_frac(double x, int &i, double &f)
+{
+    const double t = __dadd_rd(x, 4503599627370496.0);            // 2^52 + floor(x), exact
+    i = lo32(t);
+    f = x - (t - 4503599627370496.0);
+}
+
+__device__ __forceinline__ void floor_frac1(double x, int &i, float &f1)
+{
+    const double t = __dadd_rd(x, 4503599627370496.0);            // 2^52 + floor(x), exact
+    i = lo32(t);
+    const double u = __dadd_rd(x, -(t - 4503599627370497.0));     // 1 + frac(x) in [1, 2)
+    f1 = __uint_as_float(0x3f800000u | (__funnelshift_l((unsigned)lo32(u), (unsigned)hi32(u), 3) & 0x007fffffu));
+}
 
 template <class Tab>
 __device__ __forceinline__ double2 table_node(const TableConsts &tc, const Tab &tab, int i, int j)
@@ -72,18 +87,21 @@ __device__ __forceinline__ double2 table_node(const TableConsts &tc, const Tab &
 }
 
 // Interpolated {D_rho, D_z} at (rho, az = |r_z|), rho < rho_max.
-template <int INTERP, class Tab>
-__device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Tab &tab, double rho,
+template <int INTERP>
+__device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const GlobalTable &tab, double rho,
                                                 double az)
 {
     const double xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
     if (INTERP == 0) {
-        int i0 = __double2int_rd(xr), j0 = __double2int_rd(xz);
-        const double fr = xr - (double)i0, fz = xz - (double)j0;
-        // a weight of exactly 0 multiplies the clamped node when rho or |r_z| sits on the last node
+        int i0, j0;
+        double fr, fz;
+        floor_frac(xr, i0, fr);
+        floor_frac(xz, j0, fz);
+        // a weight of exactly 0 multiplies the clamped node when rho or |r_z| sits on the last node;
+        // lanes beyond rho_max (and the padding particles) arrive here too: any node will do for them
+        i0 = min(max(i0, 0), tc.nrho - 1);
+        j0 = min(max(j0, 0), tc.nz - 1);
         const int i1 = min(i0 + 1, tc.nrho - 1), j1 = min(j0 + 1, tc.nz - 1);
-        i0 = min(i0, tc.nrho - 1);
-        j0 = min(j0, tc.nz - 1);
         const double2 d00 = tab.node(i0 * tc.nz + j0);
         const double2 d01 = tab.node(i0 * tc.nz + j1);
         const double2 d10 = tab.node(i1 * tc.nz + j0);
@@ -92,8 +110,14 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Tab
         const double ay = fma(fz, d01.y - d00.y, d00.y), by = fma(fz, d11.y - d10.y, d10.y);
         return make_double2(fma(fr, bx - ax, ax), fma(fr, by - ay, ay));
     }
-    const int ic = __double2int_rd(xr + 0.5), jc = __double2int_rd(xz + 0.5);
-    const double dr = xr - (double)ic, dz = xz - (double)jc;
+    int ic, jc;
+    double dr, dz;
+    floor_frac(xr + 0.5, ic, dr);
+    floor_frac(xz + 0.5, jc, dz);
+    dr -= 0.5;
+    dz -= 0.5;
+    ic = min(max(ic, 0), tc.nrho - 1);
+    jc = min(max(jc, 0), tc.nz - 1);
     const double wr[3] = {0.5 * (0.5 - dr) * (0.5 - dr), 0.75 - dr * dr, 0.5 * (0.5 + dr) * (0.5 + dr)};
     const double wz[3] = {0.5 * (0.5 - dz) * (0.5 - dz), 0.75 - dz * dz, 0.5 * (0.5 + dz) * (0.5 + dz)};
     double ox = 0.0, oy = 0.0;
@@ -112,35 +136,88 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Tab
     return make_double2(ox, oy);
 }
 
-// -f of one pair (see the header): (px, py, pz).
-template <int INTERP, class Tab>
-__device__ __forceinline__ void table_pair(double rx, double ry, double rz, double hi, double hj,
-                                           int soft_hi, const TableConsts &tc, const Tab &tab,
-                                           double &px, double &py, double &pz)
+// Copy of the float table in shared memory with a one-node halo on every side, filled by the boundary rules
+// (D_rho odd in rho / even in z, D_z even in rho / odd in z about z = 0 and z = L/2, clamped beyond
+// rho_max): node (i, j), -1 <= i <= nrho, -1 <= j <= nz, sits at s_table[(i + 1) * (nz + 2) + j + 1], so
+// neither interpolation needs an index clamp, a reflection or a sign.
+__host__ __device__ inline size_t table_halo_nodes(int nrho, int nz) { return (size_t)(nrho + 2) * (nz + 2); }
+
+__device__ __forceinline__ void stage_table_halo(float2 *s_table, const float2 *__restrict__ table_f32,
+                                                 int nrho, int nz, int nthreads)
 {
-    const double rho2 = fma(ry, ry, rx * rx);
-    // rho2 == 0: y = 0 kills the radial table term (D_rho(0) = 0 and no direction)
-    const double y = (rho2 > 0.0) ? rsqrt_full(rho2) : 0.0;
-    if (rho2 < tc.rho_max2) {
-        const double q = fma(rz, rz, rho2);
-        double w0 = inv_cube_sqrt(q);
-        if (hi32(q) <= soft_hi) {
-            const double hh = hi + hj;
-            if (q < hh * hh) w0 = spline_w(q, hh);
-        }
-        const double2 Dv = table_lookup<INTERP>(tc, tab, rho2 * y, fabs(rz));
-        const double cr = fma(-Dv.x, y, w0);               // w0 - D_rho / rho
-        px = cr * rx;
-        py = cr * ry;
-        pz = fma(w0, rz, (rz < 0.0) ? Dv.y : -Dv.y);       // w0 r_z - sign(r_z) D_z;  D_z(rho, 0) = 0
-    } else {
-        const double cr = tc.two_over_L * y * y;
-        px = cr * rx;
-        py = cr * ry;
-        pz = 0.0;
+    const int nzs = nz + 2, total = (nrho + 2) * nzs;
+    for (int q = threadIdx.x; q < total; q += nthreads) {
+        int i = q / nzs - 1, j = q % nzs - 1;
+        float sr = 1.0f, sz = 1.0f;
+        if (i < 0) { i = -i; sr = -1.0f; }
+        if (i > nrho - 1) i = nrho - 1;
+        if (j < 0) { j = -j; sz = -1.0f; }
+        if (j > nz - 1) { j = 2 * (nz - 1) - j; sz = -sz; }
+        const float2 v = table_f32[i * nz + j];
+        s_table[q] = make_float2(sr * v.x, sz * v.y);
     }
 }
 
+// The float table in shared memory: node indices and weights from the fp64 (rho, |r_z|), the weighted sum
+// of the float nodes in fp32 (its rounding, ~1e-7 of D, is of the size of the nodes' own), two conversions.
+template <int INTERP>
+__device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const SharedTableF32 &tab,
+                                                double rho, double az)
+{
+    const float2 *D = tab.D;
+    const int nzs = tc.nz + 2;
+    float ox, oy;
+    if (INTERP == 0) {
+        int i0, j0;
+        float fr1, fz1;
+        floor_frac1(rho * tc.inv_drho, i0, fr1);
+        floor_frac1(az * tc.inv_dz, j0, fz1);
+        const float fr = fr1 - 1.0f, fz = fz1 - 1.0f;
+        // lanes beyond rho_max (and the padding particles) arrive here too: any node will do for them
+        // (j0 is in range for finite input; the clamp keeps a NaN coordinate from reading out of bounds)
+        i0 = min(max(i0, 0), tc.nrho - 1);
+        j0 = min(max(j0, 0), tc.nz - 1);
+        const float2 *d = D + (i0 + 1) * nzs + j0 + 1;
+        const float2 d00 = d[0], d01 = d[1], d10 = d[nzs], d11 = d[nzs + 1];
+        const float ax = fmaf(fz, d01.x - d00.x, d00.x), bx = fmaf(fz, d11.x - d10.x, d10.x);
+        const float ay = fmaf(fz, d01.y - d00.y, d00.y), by = fmaf(fz, d11.y - d10.y, d10.y);
+        ox = fmaf(fr, bx - ax, ax);
+        oy = fmaf(fr, by - ay, ay);
+    } else {
+        int ic, jc;
+        float fr1, fz1;
+        floor_frac1(fma(rho, tc.inv_drho, 0.5), ic, fr1);
+        floor_frac1(fma(az, tc.inv_dz, 0.5), jc, fz1);
+        const float dr = fr1 - 1.5f, dz = fz1 - 1.5f;
+        ic = min(max(ic, 0), tc.nrho - 1);
+        jc = min(max(jc, 0), tc.nz - 1);
+        const float2 *d = D + ic * nzs + jc;                 // node (ic - 1, jc - 1)
+        const float wr[3] = {0.5f * (0.5f - dr) * (0.5f - dr), 0.75f - dr * dr, 0.5f * (0.5f + dr) * (0.5f + dr)};
+        const float wz[3] = {0.5f * (0.5f - dz) * (0.5f - dz), 0.75f - dz * dz, 0.5f * (0.5f + dz) * (0.5f + dz)};
+        ox = oy = 0.0f;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float rx = 0.0f, ry = 0.0f;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const float2 v = d[a * nzs + b];
+                rx = fmaf(wz[b], v.x, rx);
+                ry = fmaf(wz[b], v.y, ry);
+            }
+            ox = fmaf(wr[a], rx, ox);
+            oy = fmaf(wr[a], ry, oy);
+        }
+    }
+    return make_double2((double)ox, (double)oy);
+}
+
+// One ring pass.  Per source the R pairs go through three phases so that the long part is one
+// branch-free block the scheduler can interleave across the R targets (with one 16-warp CTA per SM
+// there are only four warps per scheduler to hide the FP64 latencies):
+//   1. geometry, unsoftened w0 = q^-3/2, 1/rho, and the table lookup -- no branches when the table is in
+//      shared memory: lanes beyond rho_max look up a clamped node and discard it;
+//   2. the spline correction of w0 (rare; also takes the coincident / self pair q = 0);
+//   3. -f of the pair (see the header) by selects, and the accumulation.
 template <int INTERP, int R, bool SYM, class Tab>
 __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const int (&soft_hi)[R],
                                                    const SymSrc *s_src, int lane,
@@ -156,12 +233,38 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
         const double2 pa = *reinterpret_cast<const double2 *>(&sj->x);
         const double2 pb = *reinterpret_cast<const double2 *>(&sj->z);
         const double hj = sj->h;
+        double rx[R], ry[R], rz[R], q[R], w0[R], y[R];
+        double2 Dv[R];
+        bool near[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
-            const double rz = nearest_image_exact(ti[r].z - pb.x, k);
-            double px, py, pz;
-            table_pair<INTERP>(rx, ry, rz, ti[r].h, hj, soft_hi[r], tc, tab, px, py, pz);
+            rx[r] = ti[r].x - pa.x;
+            ry[r] = ti[r].y - pa.y;
+            rz[r] = nearest_image_exact(ti[r].z - pb.x, k);
+            const double rho2 = fma(ry[r], ry[r], rx[r] * rx[r]);
+            // rho2 == 0: y = 0 kills the radial table term (D_rho(0) = 0 and no direction)
+            const double yy = rsqrt_full((rho2 > 0.0) ? rho2 : 1.0);
+            y[r] = (rho2 > 0.0) ? yy : 0.0;
+            near[r] = rho2 < tc.rho_max2;
+            q[r] = fma(rz[r], rz[r], rho2);
+            w0[r] = inv_cube_sqrt(q[r]);
+            if (Tab::kLookupAlways || near[r]) Dv[r] = table_lookup<INTERP>(tc, tab, rho2 * y[r], fabs(rz[r]));
+            else Dv[r] = make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (hi32(q[r]) <= soft_hi[r]) {
+                const double hh = ti[r].h + hj;
+                if (q[r] < hh * hh) w0[r] = spline_w(q[r], hh);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double cn = fma(-Dv[r].x, y[r], w0[r]);                 // w0 - D_rho / rho
+            const double cf = tc.two_over_L * y[r] * y[r];                // line mass beyond rho_max
+            const double zn = fma(w0[r], rz[r], (rz[r] < 0.0) ? Dv[r].y : -Dv[r].y);   // D_z(rho, 0) = 0
+            const double cr = near[r] ? cn : cf;
+            const double px = cr * rx[r], py = cr * ry[r], pz = near[r] ? zn : 0.0;
             a[r][0] = fma(pb.y, px, a[r][0]);
             a[r][1] = fma(pb.y, py, a[r][1]);
             a[r][2] = fma(pb.y, pz, a[r][2]);
@@ -185,7 +288,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
 // tb + (w/4) * SYM_R + r -- and streams 128-source tiles.  grid = (n_tiles / tiles_per_cta, chunks).
 //   SMEM_TABLE = false: TW = 4, the table is read from global memory (double2 nodes);
 //   SMEM_TABLE = true : TW = 16 (one CTA per SM), the float2 table is copied to shared memory first,
-//                       dynamic shared memory = TW*3*128*8 bytes of accumulators + nodes * 8 bytes.
+//                       dynamic shared memory = TW*3*128*8 bytes of accumulators + (nrho+2)(nz+2) * 8 bytes.
 // The spline pre-test needs no restriction on max(h): only the nearest image is evaluated here.
 template <int INTERP, int TW, bool SMEM_TABLE>
 __global__ void __launch_bounds__(TW * 32, SMEM_TABLE ? 1 : 4)
@@ -205,10 +308,7 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
     double (*s_b)[3][PAIR_THREADS] = reinterpret_cast<double (*)[3][PAIR_THREADS]>(s_dyn);
     float2 *s_table = reinterpret_cast<float2 *>(s_dyn + TW * 3 * PAIR_THREADS);
 
-    if (SMEM_TABLE) {
-        const int nodes = tc.nrho * tc.nz;
-        for (int q = threadIdx.x; q < nodes; q += TW * 32) s_table[q] = table_f32[q];
-    }
+    if (SMEM_TABLE) stage_table_halo(s_table, table_f32, tc.nrho, tc.nz, TW * 32);
     GlobalTable gtab{tc.D};
     SharedTableF32 stab{s_table};
 

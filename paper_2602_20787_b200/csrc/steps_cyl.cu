@@ -416,14 +416,15 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         if (rc != STEPS_OK) return fail(rc);
         if (pp.tab_fp32) {
             // table rounded to float and staged in shared memory by a 512-thread CTA per SM
-            ctx->table_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(double) + nodes * sizeof(float2);
+            const size_t halo_bytes = table_halo_nodes(pp.tab_nrho, pp.tab_nz) * sizeof(float2);
+            ctx->table_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(double) + halo_bytes;
             if (ctx->table_smem_bytes + sizeof(SymSrc) * PAIR_THREADS > (size_t)prop.sharedMemPerBlockOptin)
                 return fail(STEPS_EUNSUPPORTED);
             std::vector<float> Df(nodes * 2);
             for (size_t q = 0; q < nodes * 2; ++q) Df[q] = (float)D[q];
             A(dev_alloc(&ctx->d_table_f32, nodes));
             if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table_f32, Df.data(), nodes * sizeof(float2), cudaMemcpyHostToDevice));
-            ctx->table_mixed_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(float) + nodes * sizeof(float2);
+            ctx->table_mixed_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(float) + halo_bytes;
             ctx->tcf.nrho = pp.tab_nrho;
             ctx->tcf.nz = pp.tab_nz;
             ctx->tcf.rho_max2 = (float)(pp.tab_rho_max * pp.tab_rho_max);

@@ -33,6 +33,10 @@ def rel_err(g, ref):
     return np.linalg.norm(g - ref, axis=1) / np.linalg.norm(ref, axis=1)
 
 
+# tab_fp32 (float nodes, fp32 weighted sum) against the oracle interpolating the same float nodes in double
+FP32_TABLE_MAX, FP32_TABLE_MEDIAN = 2e-6, 5e-8
+
+
 @pytest.mark.parametrize("interp", [0, 1])
 @pytest.mark.parametrize("cfg,n", [(0, 2048), (1, 6000)])
 def test_table_mode_matches_oracle(torch_cuda, oracle, interp, cfg, n):
@@ -104,8 +108,10 @@ def test_table_mode_tracks_the_many_image_sum(torch_cuda):
 @pytest.mark.parametrize("interp", [0, 1])
 def test_table_mode_fp32_table_in_shared_memory(torch_cuda, oracle, interp):
     """tab_fp32 = 1: the nodes are rounded to float and held in shared memory (512-thread CTAs, eight
-    target tiles each).  The oracle gets ITS table rounded the same way; all arithmetic stays double.
-    Ragged N (not a multiple of 1024) and pairs beyond rho_max included."""
+    target tiles each); node indices and weights come from the fp64 coordinates, the weighted sum of the
+    float nodes is taken in fp32, everything else stays double.  The oracle gets ITS table rounded the
+    same way and interpolates in double.  Ragged N (not a multiple of 1024) and pairs beyond rho_max
+    included."""
     from paper_2602_20787_b200 import workloads
     w = workloads.make(1, n=7001, seed=31)
     nrho, nz, rmax = 144, 128, 5.0 * w.Lz
@@ -113,11 +119,11 @@ def test_table_mode_fp32_table_in_shared_memory(torch_cuda, oracle, interp):
     D32 = D.astype(np.float32).astype(np.float64)
     ref = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D32, rmax, interp)
     g = gpu_accel_table(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, interp=interp, tab_fp32=1)
-    # a node whose double value sits within 1e-12 of a float rounding boundary may round differently on
-    # the two sides (one float ulp, 6e-8 of that node); diluted over the ~18000 nodes a particle's pairs
-    # touch this stays far below the bar
-    assert rel_err(g, ref).max() <= 1e-10
-    # and the float table changes the answer itself only at the 1e-8 level
+    # fp32 interpolation: at most ~4 float roundings (2.4e-7) of each pair's D, uncorrelated between pairs;
+    # a particle's relative error is that times sqrt(sum D^2)/|sum|, largest where the sum nearly cancels
+    e = rel_err(g, ref)
+    assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN, (e.max(), np.median(e))
+    # and the float table + float interpolation change the answer itself only at this level
     ref64 = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, interp)
     assert rel_err(g, ref64).max() <= 1e-6
 
@@ -165,7 +171,8 @@ def test_table_mode_randomised_parameters(torch_cuda, oracle, seed):
     ref32 = oracle.accel_table(x, y, z, m, h, L, G, D32, rmax, interp)
     g = gpu_accel_table(torch_cuda, (x, y, z, m, h), L, G, tab_nrho=nrho, tab_nz=nz, tab_rho_max=rmax,
                         interp=interp, ew_alpha=alpha, tab_fp32=1)
-    assert rel_err(g, ref32).max() <= 1e-10
+    e = rel_err(g, ref32)
+    assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN, (e.max(), np.median(e))
     from paper_2602_20787_b200 import binding as b
     g = gpu_accel_table(torch_cuda, (x, y, z, m, h), L, G, tab_nrho=nrho, tab_nz=nz, tab_rho_max=rmax,
                         interp=interp, ew_alpha=alpha, precision=b.PREC_MIXED)
