@@ -44,13 +44,17 @@ KERNEL_MIX = {
     # STEPS_FLAG_ORDERED_PAIRS, pair_fp64_kernel<5,0>: one ordered pair per iteration
     "fp64_ord": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
                      per_image=(9.5, 14.0)),
-    # --periodic table: pair_table_sym_kernel<CIC> (softened nearest image + 4 table gathers), one
-    # unordered pair per iteration; independent of n_cut
-    "table": dict(kernel="pair_table_sym_kernel<CIC>", interactions=2, dfma=22, dmul=14, dadd=14, dsetp=5,
+    # --periodic table: pair_table_sym_kernel<CIC, 4, false> (softened nearest image + 4 gathers of double2
+    # nodes through L1), one unordered pair per iteration; independent of n_cut
+    "table": dict(kernel="pair_table_sym_kernel<CIC>", interactions=2, dfma=23, dmul=13, dadd=17, dsetp=4,
                   per_image=(0.0, 0.0)),
+    # --periodic table --table-fp32: pair_table_sym_kernel<CIC, 16, true> (float nodes in shared memory,
+    # their weighted sum in fp32: 8 FADD + 6 FFMA per pair, not counted as FP64 work)
+    "table_f32": dict(kernel="pair_table_sym_kernel<CIC,fp32 nodes>", interactions=2, dfma=17, dmul=13, dadd=11,
+                      dsetp=3, per_image=(0.0, 0.0)),
     # --periodic table --precision mixed: pair_table_mixed_sym_kernel<CIC>, one unordered pair per iteration
-    "mixed_table": dict(kernel="pair_table_mixed_sym_kernel<CIC>", interactions=2, ffma=18, fmul=11, fadd=19,
-                        mufu=2, f2f=2, dadd=0),
+    "mixed_table": dict(kernel="pair_table_mixed_sym_kernel<CIC>", interactions=2, ffma=19, fmul=10, fadd=23,
+                        mufu=2, f2f=0, dadd=0),
     # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
     # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
     # (main loop: 38 FFMA2 + 19 FMUL2 + 16 FADD2 + 20 MUFU per ring step of two unordered pairs; counted
@@ -81,7 +85,7 @@ def pipe_counts(mode, n_cut):
         return (instr + 7.5 * d) / mix["interactions"], (flops + 9.0 * d) / mix["interactions"]
     instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
     flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
-    d = 0 if mode == "table" else 2 * (n_cut - 5)        # extra image terms per pair evaluation
+    d = 0 if mode.startswith("table") else 2 * (n_cut - 5)   # extra image terms per pair evaluation
     instr += mix["per_image"][0] * d
     flops += mix["per_image"][1] * d
     return instr / mix["interactions"], flops / mix["interactions"]
@@ -318,7 +322,7 @@ def run_ours(args):
         return
     peaks, peaks_kind = load_peaks()
     if table:
-        mode = "mixed_table" if prec == b.PREC_MIXED else "table"
+        mode = "mixed_table" if prec == b.PREC_MIXED else ("table_f32" if args.table_fp32 else "table")
     else:
         mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
         if args.ordered:
@@ -348,6 +352,12 @@ def run_ours(args):
         "pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
         "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
     }
+    if table and args.interp == "tsc":
+        # the instruction tallies above are those of the CIC loops; the TSC loops (9 gathers) are not tallied
+        roofline["kernel"] = roofline["kernel"].replace("CIC", "TSC")
+        for key in ("achieved", "frac", "flops_per_pair_interaction", "pipe_instr_per_pair_interaction",
+                    "pipe_util_vs_nominal"):
+            roofline[key] = None
     if is_mixed:
         xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
         mufu = ((KERNEL_MIX[mode]["mufu"] if table else 2 * args.n_cut) + KERNEL_MIX[mode]["f2f"]) \
@@ -355,7 +365,8 @@ def run_ours(args):
         roofline["xu_pipe_util_vs_nominal"] = mufu * pairs_per_step / t_pair / xu_peak
     else:
         roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
-        roofline["pipe_util_vs_measured_dfma"] = instr * pairs_per_step / t_pair / dfma_per_s
+        roofline["pipe_util_vs_measured_dfma"] = (None if roofline["frac"] is None
+                                                  else instr * pairs_per_step / t_pair / dfma_per_s)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle

@@ -98,8 +98,9 @@ __device__ __forceinline__ void ring_subtile_table_f32(const MixTgt (&ti)[R], co
             // exact nearest image: |rz| <= L/2 afterwards
             const float sg = (fabsf(rz0) > k.halfL) ? copysignf(1.0f, rz0) : 0.0f;
             rz[r] = fmaf(-sg, k.Ll, fmaf(-sg, k.Lh, rz0));
-            const float rho2 = fmaf(ry[r], ry[r], rx[r] * rx[r]);
-            y[r] = (rho2 > 0.0f) ? rsqrt_f32(rho2) : 0.0f;
+            // + 1e-36: keeps 1/rho finite for rho = 0 (see ring_subtile_table)
+            const float rho2 = fmaf(ry[r], ry[r], fmaf(rx[r], rx[r], 1.0e-36f));
+            y[r] = rsqrt_f32(rho2);
             near[r] = rho2 < tc.rho_max2;
             q[r] = fmaf(rz[r], rz[r], rho2);
             w0[r] = inv_cube_sqrt_f32(q[r]);
@@ -116,7 +117,8 @@ __device__ __forceinline__ void ring_subtile_table_f32(const MixTgt (&ti)[R], co
         for (int r = 0; r < R; ++r) {
             const float cn = fmaf(-Dv[r].x, y[r], w0[r]);
             const float cf = tc.two_over_L * y[r] * y[r];
-            const float zn = fmaf(w0[r], rz[r], (rz[r] < 0.0f) ? Dv[r].y : -Dv[r].y);
+            const float dz = __int_as_float(__float_as_int(Dv[r].y) ^ (~__float_as_int(rz[r]) & 0x80000000));
+            const float zn = fmaf(w0[r], rz[r], dz);           // w0 r_z - sign(r_z) D_z
             const float cr = near[r] ? cn : cf;
             const float px = cr * rx[r], py = cr * ry[r], pz = near[r] ? zn : 0.0f;
             a[r][0] = fmaf(jh.w, px, a[r][0]);

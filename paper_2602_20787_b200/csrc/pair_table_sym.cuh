@@ -241,10 +241,10 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
             rx[r] = ti[r].x - pa.x;
             ry[r] = ti[r].y - pa.y;
             rz[r] = nearest_image_exact(ti[r].z - pb.x, k);
-            const double rho2 = fma(ry[r], ry[r], rx[r] * rx[r]);
-            // rho2 == 0: y = 0 kills the radial table term (D_rho(0) = 0 and no direction)
-            const double yy = rsqrt_full((rho2 > 0.0) ? rho2 : 1.0);
-            y[r] = (rho2 > 0.0) ? yy : 0.0;
+            // + 1e-300 (below half an ulp of any rho^2 that matters): keeps 1/rho finite for rho = 0, where
+            // the interpolated D_rho underflows to D_rho(0) = 0 and (r_x, r_y) = 0 removes the direction
+            const double rho2 = fma(ry[r], ry[r], fma(rx[r], rx[r], 1.0e-300));
+            y[r] = rsqrt_full(rho2);
             near[r] = rho2 < tc.rho_max2;
             q[r] = fma(rz[r], rz[r], rho2);
             w0[r] = inv_cube_sqrt(q[r]);
@@ -262,7 +262,9 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
         for (int r = 0; r < R; ++r) {
             const double cn = fma(-Dv[r].x, y[r], w0[r]);                 // w0 - D_rho / rho
             const double cf = tc.two_over_L * y[r] * y[r];                // line mass beyond rho_max
-            const double zn = fma(w0[r], rz[r], (rz[r] < 0.0) ? Dv[r].y : -Dv[r].y);   // D_z(rho, 0) = 0
+            // w0 r_z - sign(r_z) D_z: the sign of D_z flipped unless r_z < 0, on the high word (D_z(rho, 0) = 0)
+            const double dz = __hiloint2double(hi32(Dv[r].y) ^ (~hi32(rz[r]) & 0x80000000), lo32(Dv[r].y));
+            const double zn = fma(w0[r], rz[r], dz);
             const double cr = near[r] ? cn : cf;
             const double px = cr * rx[r], py = cr * ry[r], pz = near[r] ? zn : 0.0;
             a[r][0] = fma(pb.y, px, a[r][0]);
