@@ -352,6 +352,8 @@ def run_ours(args):
         "pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
         "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
     }
+    if table and args.deterministic:                       # same loops, scheduled in rounds (pair_table_round.cuh)
+        roofline["kernel"] = roofline["kernel"].replace("sym_kernel", "round_kernel")
     if table and args.interp == "tsc":
         # the instruction tallies above are those of the CIC loops; the TSC loops (9 gathers) are not tallied
         roofline["kernel"] = roofline["kernel"].replace("CIC", "TSC")

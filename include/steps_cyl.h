@@ -56,7 +56,7 @@ typedef enum {
     STEPS_ECUDA        = -3,  /* a CUDA runtime call failed (or no device present)                     */
     STEPS_ENOMEM       = -4,  /* host or device allocation failed                                      */
     STEPS_EUNSUPPORTED = -5   /* a combination this build does not contain (EWALD_TABLE with
-                                 STEPS_FLAG_DETERMINISTIC, or a float table too large for shared memory) */
+                                 STEPS_FLAG_ORDERED_PAIRS, or a float table too large for shared memory) */
 } steps_cyl_status;
 
 enum { STEPS_PERIODIC_IMAGES = 0,      /* Eq. 8, truncated image sum                                  */
@@ -73,8 +73,8 @@ enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz             
 enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default kernels evaluate every
                                           unordered pair once and add it to both particles with
                                           floating-point atomics (same terms, summation order varies from
-                                          run to run, ~1e-16).  With this flag the images mode
-                                          schedules the same evaluation in conflict-free rounds with
+                                          run to run, ~1e-16).  With this flag both periodic modes
+                                          schedule the same evaluation in conflict-free rounds with
                                           plain stores (~3 % slower)                                    */
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,

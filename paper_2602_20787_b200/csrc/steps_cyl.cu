@@ -18,6 +18,7 @@
 #include "pair_mixed_sym.cuh"
 #include "pair_table_sym.cuh"
 #include "pair_table_mixed_sym.cuh"
+#include "pair_table_round.cuh"
 #include "ewald_table.h"
 
 using namespace steps;
@@ -187,8 +188,47 @@ void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
                                                            c->part);
 }
 
+// EWALD_TABLE + DETERMINISTIC: one launch per round (pair_table_round.cuh).
+void launch_table_rounds(steps_cyl_ctx *c, cudaStream_t s)
+{
+    const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1), groups = T / SYM_R;
+    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad;
+    const bool cic = c->tc.interp == STEPS_INTERP_CIC;
+    const int g16 = std::min(c->sm_count, (groups + 3) / 4), g4 = std::min(groups, 8 * c->sm_count);
+    const size_t sb4 = 4 * 3 * PAIR_THREADS * sizeof(double);
+    for (int r = 0; r <= last; ++r) {
+        if (c->p.precision == STEPS_PREC_MIXED) {
+            if (cic)
+                pair_table_mixed_round_kernel<0><<<g16, 512, c->table_mixed_smem_bytes, s>>>(
+                    c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->mc, c->tcf, c->d_table_f32, acc_i, acc_j);
+            else
+                pair_table_mixed_round_kernel<1><<<g16, 512, c->table_mixed_smem_bytes, s>>>(
+                    c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->mc, c->tcf, c->d_table_f32, acc_i, acc_j);
+        } else if (c->d_table_f32) {
+            if (cic)
+                pair_table_round_kernel<0, 16, true><<<g16, 512, c->table_smem_bytes, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->kc, c->tc, c->d_table_f32, acc_i, acc_j);
+            else
+                pair_table_round_kernel<1, 16, true><<<g16, 512, c->table_smem_bytes, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->kc, c->tc, c->d_table_f32, acc_i, acc_j);
+        } else {
+            if (cic)
+                pair_table_round_kernel<0, 4, false><<<g4, PAIR_THREADS, sb4, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->kc, c->tc, nullptr, acc_i, acc_j);
+            else
+                pair_table_round_kernel<1, 4, false><<<g4, PAIR_THREADS, sb4, s>>>(
+                    c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->kc, c->tc, nullptr, acc_i, acc_j);
+        }
+    }
+    c->launches += last + 1;
+}
+
 void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
+    if (c->table_mode && c->use_rounds) {
+        launch_table_rounds(c, s);
+        return;
+    }
     if (c->table_mode) {
         dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
         const size_t sb4 = 4 * 3 * PAIR_THREADS * sizeof(double);
@@ -273,7 +313,7 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
     ctx->ev_valid = true;
     finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
                                                          ctx->use_sym ? 1 : (ctx->use_rounds ? 2 : ctx->n_chunks),
-                                                         ctx->table_mode ? 1 : ctx->n_chunks,
+                                                         ctx->table_mode ? (ctx->use_rounds ? 2 : 1) : ctx->n_chunks,
                                                          ctx->kc.halfL, ctx->flags,
                                                          ctx->p.G, ctx->p.Lz, gx, gy, gz);
     ctx->launches += 1;
@@ -327,7 +367,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             !(pp.tab_rho_max > 0.0) || !std::isfinite(pp.tab_rho_max) ||
             (pp.interp != STEPS_INTERP_CIC && pp.interp != STEPS_INTERP_TSC))
             return STEPS_EINVAL;
-        if (p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS)) return STEPS_EUNSUPPORTED;
+        if (p->flags & STEPS_FLAG_ORDERED_PAIRS) return STEPS_EUNSUPPORTED;
         if (p->precision == STEPS_PREC_MIXED) pp.tab_fp32 = 1;      // mixed mode always uses the float table
     }
 
@@ -354,8 +394,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
     ctx->use_sym = !(p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS));
-    ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS) &&
-                      p->periodic_mode == STEPS_PERIODIC_IMAGES;
+    ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS);
 
     const double L = p->Lz;
     ctx->kc.L = L;
@@ -418,7 +457,9 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             // table rounded to float and staged in shared memory by a 512-thread CTA per SM
             const size_t halo_bytes = table_halo_nodes(pp.tab_nrho, pp.tab_nz) * sizeof(float2);
             ctx->table_smem_bytes = 16 * 3 * PAIR_THREADS * sizeof(double) + halo_bytes;
-            if (ctx->table_smem_bytes + sizeof(SymSrc) * PAIR_THREADS > (size_t)prop.sharedMemPerBlockOptin)
+            // static shared memory: one source tile (four, one per quad, in the round-scheduled kernels)
+            if (ctx->table_smem_bytes + (ctx->use_rounds ? 4 : 1) * sizeof(SymSrc) * PAIR_THREADS >
+                (size_t)prop.sharedMemPerBlockOptin)
                 return fail(STEPS_EUNSUPPORTED);
             std::vector<float> Df(nodes * 2);
             for (size_t q = 0; q < nodes * 2; ++q) Df[q] = (float)D[q];
@@ -435,6 +476,10 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             A(cudaFuncSetAttribute(pair_table_mixed_sym_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
             A(cudaFuncSetAttribute(pair_table_sym_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
             A(cudaFuncSetAttribute(pair_table_sym_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_mixed_round_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_mixed_round_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_round_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
+            A(cudaFuncSetAttribute(pair_table_round_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
             if (rc != STEPS_OK) return fail(rc);
         }
         ctx->tc.D = ctx->d_table;
@@ -669,7 +714,7 @@ const char *steps_cyl_strerror(int code)
     case STEPS_ESOFT: return "softening precondition violated (some h_i <= 0)";
     case STEPS_ECUDA: return "CUDA runtime error (see steps_cyl_last_cuda_error)";
     case STEPS_ENOMEM: return "out of memory";
-    case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE with the DETERMINISTIC flag, or a float table too large for shared memory)";
+    case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE with the ORDERED_PAIRS flag, or a float table too large for shared memory)";
     default: return "unknown status";
     }
 }

@@ -23,6 +23,8 @@ def main():
     ap.add_argument("--configs", default="0,1,2,3,4")
     ap.add_argument("--targets", type=int, default=256)
     ap.add_argument("--n", type=int, default=0, help="override N (debugging)")
+    ap.add_argument("--table", action="store_true",
+                    help="also EWALD_TABLE mode (144 x 128 CIC, rho_max = 5 L) against oracle.accel_table")
     args = ap.parse_args()
     import torch
     import oracle
@@ -56,6 +58,31 @@ def main():
             got = np.stack([t.cpu().numpy() for t in g], 1)
             ctx.close()
             e = np.linalg.norm(got[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
+            mom = max(abs(np.sum(w.m * got[:, c])) / np.sum(w.m * np.abs(got[:, c])) for c in range(3))
+            print("| %d | %d | %s | %d | %.2e | %.2e | %.4g | %.1e |"
+                  % (cfg, w.n, name, len(idx), e.max(), np.sqrt(np.mean(e ** 2)), secs, mom), flush=True)
+        if not args.table:
+            continue
+        # EWALD_TABLE mode: the oracle interpolates ITS table (double nodes, or the same nodes rounded to
+        # float for the two shared-memory variants) in double
+        rmax = 5.0 * w.Lz
+        D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, 144, 128, rmax)
+        D32 = D.astype(np.float32).astype(np.float64)
+        refs = {0: np.stack(oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, 0, targets=idx), 1),
+                1: np.stack(oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D32, rmax, 0, targets=idx), 1)}
+        for name, prec, f32 in (("table, double nodes (global memory)", b.PREC_FP64, 0),
+                                ("table, float nodes (shared memory)", b.PREC_FP64, 1),
+                                ("table, mixed", b.PREC_MIXED, 1)):
+            ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, precision=prec, periodic_mode=b.PERIODIC_EWALD_TABLE,
+                             tab_fp32=f32)
+            g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+            ctx.accel(*dev, *g)
+            ctx.check()
+            secs = ctx.last_pair_kernel_ms() * 1e-3
+            got = np.stack([t.cpu().numpy() for t in g], 1)
+            ctx.close()
+            ref_t = refs[f32]
+            e = np.linalg.norm(got[idx] - ref_t, axis=1) / np.linalg.norm(ref_t, axis=1)
             mom = max(abs(np.sum(w.m * got[:, c])) / np.sum(w.m * np.abs(got[:, c])) for c in range(3))
             print("| %d | %d | %s | %d | %.2e | %.2e | %.4g | %.1e |"
                   % (cfg, w.n, name, len(idx), e.max(), np.sqrt(np.mean(e ** 2)), secs, mom), flush=True)

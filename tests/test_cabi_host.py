@@ -54,7 +54,7 @@ def test_init_rejects_bad_arguments(lib):
         assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EINVAL, bad
         assert not ctx.value
     # EWALD_TABLE has no ordered-pair kernel; bad table parameters are EINVAL
-    for extra in (dict(flags=b.FLAG_DETERMINISTIC),):
+    for extra in (dict(flags=b.FLAG_ORDERED_PAIRS), dict(flags=b.FLAG_ORDERED_PAIRS | b.FLAG_DETERMINISTIC)):
         p = b.Params(**{**good, "periodic_mode": b.PERIODIC_EWALD_TABLE, **extra})
         assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EUNSUPPORTED
     for extra in (dict(tab_nrho=1), dict(ew_alpha=-1.0), dict(interp=5), dict(tab_rho_max=-3.0), dict(tab_fp32=2)):

@@ -222,3 +222,38 @@ def test_kdk_step_in_table_mode_is_the_same_leapfrog(torch_cuda, oracle):
     assert np.abs(gv - v).max() <= 1e-10 * np.abs(v).max()
     gg = np.stack([t.cpu().numpy() for t in g], 1)
     assert (np.linalg.norm(gg - g1, axis=1) / np.linalg.norm(g1, axis=1)).max() <= 1e-10
+
+
+@pytest.mark.parametrize("interp", [0, 1])
+@pytest.mark.parametrize("variant", ["double_global", "float_shared", "mixed"])
+def test_table_mode_deterministic_rounds(torch_cuda, oracle, variant, interp):
+    """STEPS_FLAG_DETERMINISTIC in EWALD_TABLE mode (pair_table_round.cuh): conflict-free rounds, plain stores.
+    Same bars as the atomic kernels, bit-identical between runs, and equal to the atomic kernels up to
+    the summation order.  Ragged N; n = 3000 gives 24 tiles (12 groups, 13 rounds), n = 700 one CTA."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    kw = dict(double_global=dict(), float_shared=dict(tab_fp32=1), mixed=dict(precision=b.PREC_MIXED))[variant]
+    for cfg, n in [(1, 3000), (4, 700)]:
+        w = workloads.make(cfg, n=n, seed=90 + n)
+        arrs = (w.x, w.y, w.z, w.m, w.h)
+        rmax = 5.0 * w.Lz
+        D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, 144, 128, rmax)
+        if variant != "double_global":
+            D = D.astype(np.float32).astype(np.float64)
+        ref = oracle.accel_table(*arrs, w.Lz, w.G, D, rmax, interp)
+        g1 = gpu_accel_table(torch_cuda, arrs, w.Lz, w.G, interp=interp, flags=b.FLAG_DETERMINISTIC, **kw)
+        g2 = gpu_accel_table(torch_cuda, arrs, w.Lz, w.G, interp=interp, flags=b.FLAG_DETERMINISTIC, **kw)
+        for a, c in zip(g1, g2):
+            assert np.array_equal(a, c)
+        e = rel_err(g1, ref)
+        if variant == "double_global":
+            assert e.max() <= 1e-10
+        elif variant == "float_shared":
+            assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN, (e.max(), np.median(e))
+        else:
+            assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4, (e.max(), np.sqrt(np.mean(e ** 2)))
+        ga = gpu_accel_table(torch_cuda, arrs, w.Lz, w.G, interp=interp, **kw)
+        assert rel_err(g1, ga).max() <= (1e-12 if variant != "mixed" else 1e-5)
+        # Newton's third law survives the scheduling
+        mom = max(abs(np.sum(w.m * g1[c])) / np.sum(w.m * np.abs(g1[c])) for c in range(3))
+        assert mom <= (1e-13 if variant != "mixed" else 1e-6)
