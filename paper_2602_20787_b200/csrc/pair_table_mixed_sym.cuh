@@ -26,7 +26,7 @@ __device__ __forceinline__ void floor_frac_f32(float x, int &i, float &f)
 // Interpolated {D_rho, D_z} in float; nodes from the shared-memory float2 table.
 template <int INTERP>
 __device__ __forceinline__ float2 table_lookup_f32(const TableConstsF32 &tc, const float2 *tab, float rho,
-                                                  float az)
+                                                  float az, bool live)
 {
     const float xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
     const int nzs = tc.nz + 2;
@@ -38,7 +38,8 @@ __device__ __forceinline__ float2 table_lookup_f32(const TableConstsF32 &tc, con
         // lanes beyond rho_max (and the padding particles) arrive here too: any node will do for them
         i0 = min(max(i0, 0), tc.nrho - 1);
         j0 = min(max(j0, 0), tc.nz - 1);
-        const float2 *d = tab + (i0 + 1) * nzs + j0 + 1;    // haloed table: stage_table_halo()
+        // haloed table (stage_table_halo); lanes whose value is discarded all read node (-1, -1): a broadcast
+        const float2 *d = tab + (live ? (i0 + 1) * nzs + j0 + 1 : 0);
         const float2 d00 = d[0], d01 = d[1], d10 = d[nzs], d11 = d[nzs + 1];
         const float ax = fmaf(fz, d01.x - d00.x, d00.x), bx = fmaf(fz, d11.x - d10.x, d10.x);
         const float ay = fmaf(fz, d01.y - d00.y, d00.y), by = fmaf(fz, d11.y - d10.y, d10.y);
@@ -52,7 +53,7 @@ __device__ __forceinline__ float2 table_lookup_f32(const TableConstsF32 &tc, con
     dz -= 0.5f;
     ic = min(max(ic, 0), tc.nrho - 1);
     jc = min(max(jc, 0), tc.nz - 1);
-    const float2 *d = tab + ic * nzs + jc;                  // node (ic - 1, jc - 1)
+    const float2 *d = tab + (live ? ic * nzs + jc : 0);     // node (ic - 1, jc - 1)
     const float wr[3] = {0.5f * (0.5f - dr) * (0.5f - dr), 0.75f - dr * dr, 0.5f * (0.5f + dr) * (0.5f + dr)};
     const float wz[3] = {0.5f * (0.5f - dz) * (0.5f - dz), 0.75f - dz * dz, 0.5f * (0.5f + dz) * (0.5f + dz)};
     float ox = 0.0f, oy = 0.0f;
@@ -104,7 +105,7 @@ __device__ __forceinline__ void ring_subtile_table_f32(const MixTgt (&ti)[R], co
             near[r] = rho2 < tc.rho_max2;
             q[r] = fmaf(rz[r], rz[r], rho2);
             w0[r] = inv_cube_sqrt_f32(q[r]);
-            Dv[r] = table_lookup_f32<INTERP>(tc, tab, rho2 * y[r], fabsf(rz[r]));
+            Dv[r] = table_lookup_f32<INTERP>(tc, tab, rho2 * y[r], fabsf(rz[r]), near[r]);
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {

@@ -89,7 +89,7 @@ __device__ __forceinline__ double2 table_node(const TableConsts &tc, const Tab &
 // Interpolated {D_rho, D_z} at (rho, az = |r_z|), rho < rho_max.
 template <int INTERP>
 __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const GlobalTable &tab, double rho,
-                                                double az)
+                                                double az, bool /*live*/)
 {
     const double xr = rho * tc.inv_drho, xz = az * tc.inv_dz;
     if (INTERP == 0) {
@@ -162,7 +162,7 @@ __device__ __forceinline__ void stage_table_halo(float2 *s_table, const float2 *
 // of the float nodes in fp32 (its rounding, ~1e-7 of D, is of the size of the nodes' own), two conversions.
 template <int INTERP>
 __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const SharedTableF32 &tab,
-                                                double rho, double az)
+                                                double rho, double az, bool live)
 {
     const float2 *D = tab.D;
     const int nzs = tc.nz + 2;
@@ -177,6 +177,8 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Sha
         // (j0 is in range for finite input; the clamp keeps a NaN coordinate from reading out of bounds)
         i0 = min(max(i0, 0), tc.nrho - 1);
         j0 = min(max(j0, 0), tc.nz - 1);
+        // (this loop is bound by issue slots: redirecting the discarded lanes' gathers to one broadcast
+        // address, as the TSC branch does, costs more in its SEL than it saves in bank conflicts)
         const float2 *d = D + (i0 + 1) * nzs + j0 + 1;
         const float2 d00 = d[0], d01 = d[1], d10 = d[nzs], d11 = d[nzs + 1];
         const float ax = fmaf(fz, d01.x - d00.x, d00.x), bx = fmaf(fz, d11.x - d10.x, d10.x);
@@ -191,7 +193,9 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Sha
         const float dr = fr1 - 1.5f, dz = fz1 - 1.5f;
         ic = min(max(ic, 0), tc.nrho - 1);
         jc = min(max(jc, 0), tc.nz - 1);
-        const float2 *d = D + ic * nzs + jc;                 // node (ic - 1, jc - 1)
+        // node (ic - 1, jc - 1); lanes whose value is discarded all read node (-1, -1): one broadcast, no bank
+        // conflicts (the nine gathers per pair make this loop shared-memory bound)
+        const float2 *d = D + (live ? ic * nzs + jc : 0);
         const float wr[3] = {0.5f * (0.5f - dr) * (0.5f - dr), 0.75f - dr * dr, 0.5f * (0.5f + dr) * (0.5f + dr)};
         const float wz[3] = {0.5f * (0.5f - dz) * (0.5f - dz), 0.75f - dz * dz, 0.5f * (0.5f + dz) * (0.5f + dz)};
         ox = oy = 0.0f;
@@ -248,7 +252,7 @@ __device__ __forceinline__ void ring_subtile_table(const SymTgt (&ti)[R], const 
             near[r] = rho2 < tc.rho_max2;
             q[r] = fma(rz[r], rz[r], rho2);
             w0[r] = inv_cube_sqrt(q[r]);
-            if (Tab::kLookupAlways || near[r]) Dv[r] = table_lookup<INTERP>(tc, tab, rho2 * y[r], fabs(rz[r]));
+            if (Tab::kLookupAlways || near[r]) Dv[r] = table_lookup<INTERP>(tc, tab, rho2 * y[r], fabs(rz[r]), near[r]);
             else Dv[r] = make_double2(0.0, 0.0);
         }
 #pragma unroll
