@@ -257,3 +257,28 @@ def test_table_mode_deterministic_rounds(torch_cuda, oracle, variant, interp):
         # Newton's third law survives the scheduling
         mom = max(abs(np.sum(w.m * g1[c])) / np.sum(w.m * np.abs(g1[c])) for c in range(3))
         assert mom <= (1e-13 if variant != "mixed" else 1e-6)
+
+
+@pytest.mark.parametrize("variant", ["float_shared", "mixed", "float_shared_deterministic"])
+def test_table_mode_bench_size_sampled_targets(torch_cuda, oracle, variant):
+    """The table-mode configurations bench.py times (config 3 load, N = 1 048 576, 144 x 128 CIC, rho_max = 5 L,
+    same launch configuration) on sampled targets the oracle computes one by one; momentum over ALL particles."""
+    import os
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    n = int(os.environ.get("STEPS_TEST_BENCH_N", 1048576))
+    w = workloads.make(3, n=n)
+    idx = workloads.sample_targets(w.n, 128, seed=33)
+    rmax = 5.0 * w.Lz
+    D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, 144, 128, rmax).astype(np.float32).astype(np.float64)
+    ref = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D, rmax, 0, targets=idx)
+    kw = dict(float_shared=dict(tab_fp32=1), mixed=dict(precision=b.PREC_MIXED),
+              float_shared_deterministic=dict(tab_fp32=1, flags=b.FLAG_DETERMINISTIC))[variant]
+    g = gpu_accel_table(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, **kw)
+    e = rel_err([c[idx] for c in g], ref)
+    if variant == "mixed":
+        assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4, (e.max(), np.sqrt(np.mean(e ** 2)))
+    else:
+        assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN, (e.max(), np.median(e))
+    for c in g:
+        assert abs(np.sum(w.m * c)) <= (1e-11 if variant != "mixed" else 1e-5) * np.sum(w.m * np.abs(c))
