@@ -100,35 +100,57 @@ __global__ void finalize_kernel(const double *__restrict__ part, int n, int n_pa
 // The two logarithms are merged: integrand = ln{ [(w+ + L)/(w- + L)]^2 a-/a+ }.
 struct QuadNode { double Y, e, wgt; };
 
+// Quadrature sum of the nodes kq = k0, k0 + stride, ... for a particle at radius rho.
+__device__ __forceinline__ double background_nodes(double rho, double R, double Lhalf,
+                                                   const QuadNode *__restrict__ nodes, int n_nodes,
+                                                   int k0, int stride)
+{
+    const double L2 = Lhalf * Lhalf;
+    double acc = 0.0;
+    for (int kq = k0; kq < n_nodes; kq += stride) {
+        const QuadNode q = nodes[kq];
+        const double X  = sqrt(q.e * (R + q.Y));
+        // a+- = (rho +- X)^2 + Y^2  (R^2 = X^2 + Y^2): no cancellation for rho ~ R, Y ~ 0
+        const double Y2 = q.Y * q.Y, sp = rho + X, sm = rho - X;
+        const double ap = fma(sp, sp, Y2), am = fma(sm, sm, Y2);
+        if (am <= 0.0) continue;                                      // rho == R, Y == 0: measure zero
+        const double wp = sqrt(L2 + ap), wm = sqrt(L2 + am);
+        const double ratio = (wp + Lhalf) / (wm + Lhalf);
+        acc = fma(q.wgt, log(ratio * ratio * (am / ap)), acc);
+    }
+    return acc;
+}
+
+// LANES = 1: one thread per particle.  LANES = 32: one warp per particle (nodes strided over the lanes,
+// fixed-order butterfly sum) -- for small n, where one thread per particle leaves most SMs empty and the
+// 361-node loop (~120 us) would outlast the pair kernel.
+template <int LANES>
 __global__ void background_kernel(const double *__restrict__ x, const double *__restrict__ y,
                                   int n, double R, double Lhalf, double G, double rho0,
                                   int infinite, const QuadNode *__restrict__ nodes, int n_nodes,
                                   double *__restrict__ bx, double *__restrict__ by)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = tid / LANES, lane = tid % LANES;
+    if (i >= n) return;                                               // uniform over a warp when LANES == 32
     const double xv = x[i], yv = y[i];
     const double rho = sqrt(fma(xv, xv, yv * yv));
-    if (rho0 == 0.0 || rho == 0.0) { bx[i] = 0.0; by[i] = 0.0; return; }
+    if (rho0 == 0.0 || rho == 0.0) {
+        if (lane == 0) { bx[i] = 0.0; by[i] = 0.0; }
+        return;
+    }
     double Fh;
     if (infinite) {
         Fh = -2.0 * 3.141592653589793238 * G * rho0 * rho;          // Eq. 10
     } else {
-        const double L2 = Lhalf * Lhalf;
-        double acc = 0.0;
-        for (int kq = 0; kq < n_nodes; ++kq) {
-            const QuadNode q = nodes[kq];
-            const double X  = sqrt(q.e * (R + q.Y));
-            // a+- = (rho +- X)^2 + Y^2  (R^2 = X^2 + Y^2): no cancellation for rho ~ R, Y ~ 0
-            const double Y2 = q.Y * q.Y, sp = rho + X, sm = rho - X;
-            const double ap = fma(sp, sp, Y2), am = fma(sm, sm, Y2);
-            if (am <= 0.0) continue;                                  // rho == R, Y == 0: measure zero
-            const double wp = sqrt(L2 + ap), wm = sqrt(L2 + am);
-            const double ratio = (wp + Lhalf) / (wm + Lhalf);
-            acc = fma(q.wgt, log(ratio * ratio * (am / ap)), acc);
+        double acc = background_nodes(rho, R, Lhalf, nodes, n_nodes, lane, LANES);
+        if (LANES == 32) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
         }
         Fh = 2.0 * G * rho0 * acc;
     }
+    if (lane != 0) return;
     const double s = -Fh / rho;      // Eq. 11 subtracts F_h (F_h < 0): outward push
     bx[i] = s * xv;
     by[i] = s * yv;

@@ -325,9 +325,15 @@ int enqueue_background(steps_cyl_ctx *ctx, const double *x, const double *y, dou
                        cudaStream_t s)
 {
     const int tb = 128;
-    background_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(
-        x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0,
-        ctx->p.background == STEPS_BG_INFINITE, ctx->nodes, ctx->n_nodes, bx, by);
+    const bool infinite = ctx->p.background == STEPS_BG_INFINITE;
+    if (!infinite && ctx->n <= 256 * 1024)       // one warp per particle: see background_kernel
+        background_kernel<32><<<(ctx->n * 32 + tb - 1) / tb, tb, 0, s>>>(
+            x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0, 0,
+            ctx->nodes, ctx->n_nodes, bx, by);
+    else
+        background_kernel<1><<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(
+            x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0, infinite,
+            ctx->nodes, ctx->n_nodes, bx, by);
     ctx->launches += 1;
     CK(cudaGetLastError());
     return STEPS_OK;
