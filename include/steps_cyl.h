@@ -78,7 +78,7 @@ enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default
                                           plain stores (~3 % slower)                                    */
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,
-                                          per-particle error ~3e-12 instead of ~1e-14 (bar: 1e-10)     */
+                                          per-particle error <~ 2e-12 instead of ~1e-14 (bar: 1e-10)  */
        STEPS_FLAG_ORDERED_PAIRS = 4    /* fp64 / mixed images mode: the literal form of Eq. 1 -- every target
                                           sums over all its sources (ordered pairs, fixed-order reduction,
                                           bit-reproducible, ~1.9x slower than the default)             */ };
