@@ -212,7 +212,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
 // Rounds r = 0 .. min(T/2 + 1, T - 1) are launched one after the other on the stream, so every
 // accumulator receives its contributions in a fixed order: bit-reproducible results at ~97 % of the
 // atomic kernel's speed (one tile of work per CTA per launch; T/2 + 2 launches per evaluation).
-// acc_i: [4][n_pad], acc_j: [3][n_pad], both zeroed by the host before round 0.
+// acc_i: gridDim.y slabs of [4][n_pad], acc_j: [3][n_pad], all zeroed by the host before round 0.
 template <int NC>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
@@ -241,6 +241,11 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
     __shared__ SymSrc s_src[PAIR_THREADS];
     __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
 
+    // gridDim.y == 4 (small N: a round has fewer items than the GPU has schedulers): CTA y takes source
+    // sub-tile y only and adds its target-side sums into its own slab y of acc_i
+    const bool split = gridDim.y == PAIR_THREADS / 32;
+    const int js0 = split ? blockIdx.y : 0, js1 = split ? blockIdx.y + 1 : PAIR_THREADS / 32;
+    acc_i += (size_t)blockIdx.y * 4 * n_pad;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     SymTgt ti[SYM_R];
     double a[SYM_R][4];
@@ -265,7 +270,7 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
     }
     __syncthreads();
 #pragma unroll 1
-    for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+    for (int js = js0; js < js1; ++js) {
         double bx = 0.0, by = 0.0, bz = 0.0;
         const SymSrc *sub = s_src + js * 32;
         if (mode[0] == 1 && mode[1] == 1) {
@@ -291,13 +296,14 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
         s_b[w][2][jl] = bz;
     }
     __syncthreads();
+    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA took
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double v = s_b[0][c][threadIdx.x];
 #pragma unroll
         for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
         double *p = acc_j + (size_t)c * n_pad + j;            // this CTA is the tile's only writer this round
-        *p = *p - v;
+        if (mine) *p = *p - v;
     }
 #pragma unroll
     for (int r = 0; r < SYM_R; ++r) {

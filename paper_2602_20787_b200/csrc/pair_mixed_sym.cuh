@@ -381,6 +381,10 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
     __shared__ float4 s_hi[PAIR_THREADS];
     __shared__ float4 s_lo[PAIR_THREADS];
     __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    // gridDim.y == 4: one source sub-tile per CTA, own acc_i slab (see pair_fp64_round_kernel)
+    const bool split = gridDim.y == PAIR_THREADS / 32;
+    const int js0 = split ? blockIdx.y : 0, js1 = split ? blockIdx.y + 1 : PAIR_THREADS / 32;
+    acc_i += (size_t)blockIdx.y * 4 * n_pad;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     MixTgt ti[SYM_R];
     double A[SYM_R][4];
@@ -408,7 +412,7 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
     s_lo[threadIdx.x] = f_lo[j];
     __syncthreads();
 #pragma unroll 1
-    for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+    for (int js = js0; js < js1; ++js) {
         float bx = 0.0f, by = 0.0f, bz = 0.0f;
         const float4 *sh = s_hi + js * 32, *sl = s_lo + js * 32;
         if (mode[0] == 1 && mode[1] == 1) {
@@ -445,13 +449,14 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
         s_b[w][2][jl] = bz;
     }
     __syncthreads();
+    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA took
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double v = (double)s_b[0][c][threadIdx.x];
 #pragma unroll
         for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += (double)s_b[ww][c][threadIdx.x];
         double *p = acc_j + (size_t)c * n_pad + j;
-        *p = *p - v;
+        if (mine) *p = *p - v;
     }
 #pragma unroll
     for (int r = 0; r < SYM_R; ++r) {

@@ -29,6 +29,7 @@ struct steps_cyl_ctx {
     int n_chunks, tiles_per_chunk;
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
     bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
+    int round_split = 1;                          // gridDim.y of the image-mode round kernels (1 or 4)
     bool use_rounds;                              // DETERMINISTIC: round-scheduled symmetric kernels
     int sm_count;
     PairConsts kc;
@@ -149,9 +150,9 @@ template <int NC>
 void launch_pair_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
-    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad;
+    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad * c->round_split;
     for (int r = 0; r <= last; ++r)
-        pair_fp64_round_kernel<NC><<<T / SYM_R, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
+        pair_fp64_round_kernel<NC><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
                                                                     c->n_pad, T, r, c->p.n_cut, c->kc,
                                                                     c->flags, acc_i, acc_j);
     c->launches += last;      // launch_pair() adds the remaining 2
@@ -161,9 +162,9 @@ template <int NC>
 void launch_pair_mixed_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
-    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad;
+    double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad * c->round_split;
     for (int r = 0; r <= last; ++r)
-        pair_mixed_round_kernel<NC><<<T / SYM_R, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax,
+        pair_mixed_round_kernel<NC><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax,
                                                                      c->n_pad, T, r, c->p.n_cut, c->mc,
                                                                      c->kc.halfL, c->flags, acc_i, acc_j);
     c->launches += last;
@@ -307,12 +308,12 @@ int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const do
     if (ctx->use_sym)      // the symmetric kernels accumulate with atomics into part[0..4 n_pad)
         CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * sizeof(double), s));
     if (ctx->use_rounds)   // target-side sums in slab 0, source-side sums in slab 1 (its 4th row stays 0)
-        CK(cudaMemsetAsync(ctx->part, 0, 8 * (size_t)ctx->n_pad * sizeof(double), s));
+        CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * (ctx->round_split + 1) * sizeof(double), s));
     launch_pair(ctx, s);
     CK(cudaEventRecord(ctx->ev1, s));
     ctx->ev_valid = true;
     finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
-                                                         ctx->use_sym ? 1 : (ctx->use_rounds ? 2 : ctx->n_chunks),
+                                                         ctx->use_sym ? 1 : (ctx->use_rounds ? ctx->round_split + 1 : ctx->n_chunks),
                                                          ctx->table_mode ? (ctx->use_rounds ? 2 : 1) : ctx->n_chunks,
                                                          ctx->kc.halfL, ctx->flags,
                                                          ctx->p.G, ctx->p.Lz, gx, gy, gz);
@@ -402,6 +403,11 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->use_sym = !(p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS));
     ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS);
 
+    // small N: a round has n_tiles / 2 items of four warps; below ~1.5 warps per scheduler (measured break-even:
+    // N ~ 260 000) split the items by source sub-tile
+    if (ctx->use_rounds && pp.periodic_mode == STEPS_PERIODIC_IMAGES && ctx->n_tiles / SYM_R < 6 * ctx->sm_count)
+        ctx->round_split = PAIR_THREADS / 32;
+
     const double L = p->Lz;
     ctx->kc.L = L;
     ctx->kc.halfL = 0.5 * L;
@@ -433,7 +439,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->tile_hmax, (size_t)ctx->n_tiles));
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
-    A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 2)));
+    A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 5)));
     A(dev_alloc(&ctx->bx, np));
     A(dev_alloc(&ctx->by, np));
     A(dev_alloc(&ctx->flags, 1));
