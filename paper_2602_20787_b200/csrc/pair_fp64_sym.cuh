@@ -122,6 +122,10 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
     __shared__ SymSrc s_src[PAIR_THREADS];
     __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];    // per-warp source accumulators
 
+    // gridDim.z == 4 (small N: fewer tile pairs than the GPU has schedulers): CTA z takes source sub-tile z only
+    const bool split = gridDim.z == PAIR_THREADS / 32;
+    const int js0 = split ? blockIdx.z : 0, js1 = split ? blockIdx.z + 1 : PAIR_THREADS / 32;
+    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA takes
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     SymTgt ti[SYM_R];
     double a[SYM_R][4];
@@ -154,7 +158,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             }
         }
 #pragma unroll 1
-        for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+        for (int js = js0; js < js1; ++js) {
             double bx = 0.0, by = 0.0, bz = 0.0;
             const SymSrc *sub = s_src + js * 32;
             if (t >= tb + SYM_R) {
@@ -189,7 +193,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             double v = s_b[0][c][threadIdx.x];
 #pragma unroll
             for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
-            if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
+            if (mine && v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
         }
     }
 #pragma unroll

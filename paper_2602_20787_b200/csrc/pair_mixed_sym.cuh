@@ -263,6 +263,10 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
     __shared__ float4 s_lo[PAIR_THREADS];
     __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
 
+    // gridDim.z == 4 (small N): CTA z takes source sub-tile z only (see pair_fp64_sym_kernel)
+    const bool split = gridDim.z == PAIR_THREADS / 32;
+    const int js0 = split ? blockIdx.z : 0, js1 = split ? blockIdx.z + 1 : PAIR_THREADS / 32;
+    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     MixTgt ti[SYM_R];
     double A[SYM_R][4];
@@ -299,7 +303,7 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
             }
         }
 #pragma unroll 1
-        for (int js = 0; js < PAIR_THREADS / 32; ++js) {
+        for (int js = js0; js < js1; ++js) {
             float bx = 0.0f, by = 0.0f, bz = 0.0f;
             const float4 *sh = s_hi + js * 32, *sl = s_lo + js * 32;
             if (t >= tb + SYM_R) {
@@ -341,7 +345,7 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
             double v = (double)s_b[0][c][threadIdx.x];
 #pragma unroll
             for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += (double)s_b[ww][c][threadIdx.x];
-            if (v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
+            if (mine && v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
         }
     }
 #pragma unroll

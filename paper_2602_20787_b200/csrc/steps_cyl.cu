@@ -29,6 +29,7 @@ struct steps_cyl_ctx {
     int n_chunks, tiles_per_chunk;
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
     bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
+    int sym_split = 1;                            // gridDim.z of the symmetric image-mode kernels (1 or 4)
     int round_split = 1;                          // gridDim.y of the image-mode round kernels (1 or 4)
     bool use_rounds;                              // DETERMINISTIC: round-scheduled symmetric kernels
     int sm_count;
@@ -118,6 +119,8 @@ void choose_chunks(steps_cyl_ctx *c)
     tpc = std::max(1, std::min(tpc, 64));
     c->sym_tiles_per_chunk = tpc;
     c->sym_chunks = (c->n_tiles + tpc - 1) / tpc;
+    // small N: fewer (target pair, source tile) items than two per SM -> split them by source sub-tile
+    c->sym_split = (tri / SYM_R < 2.0 * c->sm_count) ? PAIR_THREADS / 32 : 1;
 }
 
 template <int NC>
@@ -132,7 +135,7 @@ void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
 template <int NC>
 void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
-    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
+    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
     if (c->p.flags & STEPS_FLAG_FAR_ORDER2)
         pair_fp64_sym_kernel<NC, true><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
                                                                     c->n_pad, c->n_tiles,
@@ -182,7 +185,7 @@ void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
 template <int NC>
 void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
-    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks);
+    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
     pair_mixed_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax, c->n_pad,
                                                            c->n_tiles, c->sym_tiles_per_chunk,
                                                            c->p.n_cut, c->mc, c->kc.halfL, c->flags,
