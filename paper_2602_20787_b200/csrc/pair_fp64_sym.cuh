@@ -217,7 +217,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
 // accumulator receives its contributions in a fixed order: bit-reproducible results at ~97 % of the
 // atomic kernel's speed (one tile of work per CTA per launch; T/2 + 2 launches per evaluation).
 // acc_i: gridDim.y slabs of [4][n_pad], acc_j: [3][n_pad], all zeroed by the host before round 0.
-template <int NC>
+template <int NC, bool SPLIT>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                        const double *__restrict__ hs, const double *__restrict__ tile_hmax,
@@ -245,11 +245,10 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
     __shared__ SymSrc s_src[PAIR_THREADS];
     __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
 
-    // gridDim.y == 4 (small N: a round has fewer items than the GPU has schedulers): CTA y takes source
+    // SPLIT (gridDim.y == 4; small N: a round has fewer items than the GPU has schedulers): CTA y takes source
     // sub-tile y only and adds its target-side sums into its own slab y of acc_i
-    const bool split = gridDim.y == PAIR_THREADS / 32;
-    const int js0 = split ? blockIdx.y : 0, js1 = split ? blockIdx.y + 1 : PAIR_THREADS / 32;
-    acc_i += (size_t)blockIdx.y * 4 * n_pad;
+    const int js0 = SPLIT ? blockIdx.y : 0, js1 = SPLIT ? blockIdx.y + 1 : PAIR_THREADS / 32;
+    if (SPLIT) acc_i += (size_t)blockIdx.y * 4 * n_pad;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     SymTgt ti[SYM_R];
     double a[SYM_R][4];
@@ -300,7 +299,7 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
         s_b[w][2][jl] = bz;
     }
     __syncthreads();
-    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA took
+    const bool mine = !SPLIT || (int)(threadIdx.x >> 5) == js0;                      // sources this CTA took
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double v = s_b[0][c][threadIdx.x];

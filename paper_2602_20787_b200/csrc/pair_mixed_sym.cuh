@@ -358,7 +358,7 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
 
 // Deterministic variant in rounds: the scheduling of pair_fp64_round_kernel (pair_fp64_sym.cuh) with the
 // float pair arithmetic of this file.  acc_i: [4][n_pad], acc_j: [3][n_pad], zeroed before round 0.
-template <int NC>
+template <int NC, bool SPLIT>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
 pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
                         const double *__restrict__ tile_hmax, int n_pad, int n_tiles, int round,
@@ -385,10 +385,9 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
     __shared__ float4 s_hi[PAIR_THREADS];
     __shared__ float4 s_lo[PAIR_THREADS];
     __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
-    // gridDim.y == 4: one source sub-tile per CTA, own acc_i slab (see pair_fp64_round_kernel)
-    const bool split = gridDim.y == PAIR_THREADS / 32;
-    const int js0 = split ? blockIdx.y : 0, js1 = split ? blockIdx.y + 1 : PAIR_THREADS / 32;
-    acc_i += (size_t)blockIdx.y * 4 * n_pad;
+    // SPLIT (gridDim.y == 4): one source sub-tile per CTA, own acc_i slab (see pair_fp64_round_kernel)
+    const int js0 = SPLIT ? blockIdx.y : 0, js1 = SPLIT ? blockIdx.y + 1 : PAIR_THREADS / 32;
+    if (SPLIT) acc_i += (size_t)blockIdx.y * 4 * n_pad;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     MixTgt ti[SYM_R];
     double A[SYM_R][4];
@@ -453,7 +452,7 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
         s_b[w][2][jl] = bz;
     }
     __syncthreads();
-    const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA took
+    const bool mine = !SPLIT || (int)(threadIdx.x >> 5) == js0;                      // sources this CTA took
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double v = (double)s_b[0][c][threadIdx.x];

@@ -154,10 +154,14 @@ void launch_pair_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
     double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad * c->round_split;
-    for (int r = 0; r <= last; ++r)
-        pair_fp64_round_kernel<NC><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
-                                                                    c->n_pad, T, r, c->p.n_cut, c->kc,
-                                                                    c->flags, acc_i, acc_j);
+    for (int r = 0; r <= last; ++r) {
+        if (c->round_split > 1)
+            pair_fp64_round_kernel<NC, true><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->flags, acc_i, acc_j);
+        else
+            pair_fp64_round_kernel<NC, false><<<T / SYM_R, PAIR_THREADS, 0, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->flags, acc_i, acc_j);
+    }
     c->launches += last;      // launch_pair() adds the remaining 2
 }
 
@@ -166,10 +170,14 @@ void launch_pair_mixed_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     const int T = c->n_tiles, last = std::min(T / 2 + 1, T - 1);
     double *acc_i = c->part, *acc_j = c->part + 4 * (size_t)c->n_pad * c->round_split;
-    for (int r = 0; r <= last; ++r)
-        pair_mixed_round_kernel<NC><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax,
-                                                                     c->n_pad, T, r, c->p.n_cut, c->mc,
-                                                                     c->kc.halfL, c->flags, acc_i, acc_j);
+    for (int r = 0; r <= last; ++r) {
+        if (c->round_split > 1)
+            pair_mixed_round_kernel<NC, true><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(
+                c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc.halfL, c->flags, acc_i, acc_j);
+        else
+            pair_mixed_round_kernel<NC, false><<<T / SYM_R, PAIR_THREADS, 0, s>>>(
+                c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc.halfL, c->flags, acc_i, acc_j);
+    }
     c->launches += last;
 }
 
