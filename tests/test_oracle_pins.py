@@ -299,3 +299,12 @@ def test_golden_two_particle_values(oracle):
         want = np.array(list(map(float, r[6:9])))
         got = oracle.pair_accel(rx, ry, rz, hh, L, 1.0, ncut)
         np.testing.assert_allclose(got, want, rtol=1e-13, atol=1e-300)
+
+
+def test_golden_two_particle_provenance():
+    """The stored values are reproduced by the committed 40-digit script (literal Eq. 8 window on the
+    raw r_z -- a different route to the image set from the oracle's wrap + sign rule)."""
+    import os, subprocess, sys
+    script = os.path.join(os.path.dirname(__file__), "golden", "make_two_particle.py")
+    r = subprocess.run([sys.executable, script, "--check"], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
