@@ -29,13 +29,20 @@ namespace steps {
 
 constexpr int PAIR_THREADS = 128;   // targets per CTA (one per thread) == sources per tile
 constexpr int MAX_NCUT_UNROLLED = 8;
+#ifndef STEPS_RT_UNROLL
+#define STEPS_RT_UNROLL 2
+#endif
+constexpr int kRtUnroll = STEPS_RT_UNROLL;      // image-loop unroll of the run-time N_cut fp64 kernels (1/2/3/4 at
+                                                // N_cut = 10: 490 / 478 / 480 / 486 ms per evaluation at N = 262144)
+constexpr int MAX_NCUT_TABLE = 64;  // run-time N_cut up to here reads its per-image constants from PairConsts
 
 struct PairConsts {
     double L;                 // period
     double halfL;
     int L_hi, L_lo, halfL_hi; // integer views of L and L/2 (ALU-pipe wrap test)
-    double c2nL[MAX_NCUT_UNROLLED + 1];   // 2 n L
-    double n2L2[MAX_NCUT_UNROLLED + 1];   // (n L)^2
+    double c2nL[MAX_NCUT_TABLE + 1];      // 2 n L
+    double n2L2[MAX_NCUT_TABLE + 1];      // (n L)^2
+    double dn[MAX_NCUT_TABLE + 1];        // n
 };
 
 struct DevFlags {             // written by pack_kernel, read by the pair kernels
@@ -149,6 +156,22 @@ __device__ __forceinline__ void image_sum(double rz, double q, double hi, double
         S += we;
         T = (NC == 1) ? copysign(we, rz) : fma(copysign((double)NC, rz), we, T);
 
+    } else if (ncut_rt <= MAX_NCUT_TABLE) {
+        // run-time N_cut: the same arithmetic as the unrolled instances, the per-image constants
+        // (uniform across the warp) indexed out of the kernel-parameter bank
+#pragma unroll 2
+        for (int n = 1; n < ncut_rt; ++n) {
+            const double B  = q + k.n2L2[n];
+            const double wp = inv_cube_sqrt_far<O2>(fma(-k.c2nL[n], rz, B));
+            const double wm = inv_cube_sqrt_far<O2>(fma(k.c2nL[n], rz, B));
+            S += wp;
+            S += wm;
+            T = fma(k.dn[n], wp - wm, T);
+        }
+        double we = inv_cube_sqrt_far<O2>(fma(-k.c2nL[ncut_rt], fabs(rz), q + k.n2L2[ncut_rt]));
+        we = rz_nonzero ? we : 0.0;
+        S += we;
+        T = fma(copysign(k.dn[ncut_rt], rz), we, T);
     } else {
         for (int n = 1; n < ncut_rt; ++n) {
             const double nL = (double)n * k.L;
@@ -165,6 +188,53 @@ __device__ __forceinline__ void image_sum(double rz, double q, double hi, double
         we = rz_nonzero ? we : 0.0;
         S += we;
         T = fma(copysign((double)ncut_rt, rz), we, T);
+    }
+}
+
+// Run-time N_cut (NC == 0) for R targets against the same source: the image loop is the OUTER loop and the
+// targets the inner one, so that one trip has 2 R independent rsqrt chains (per unroll step) in flight and reads the
+// per-image constants once.  Same arithmetic per pair as image_sum<0>; N_cut > MAX_NCUT_TABLE falls back to it.
+template <int R, bool O2>
+__device__ __forceinline__ void image_sum_rt(const double (&rz)[R], const double (&q)[R],
+                                             const double (&hi)[R], double hj, const int (&soft_hi)[R],
+                                             const PairConsts &k, int ncut_rt, double (&S)[R], double (&T)[R])
+{
+    if (ncut_rt > MAX_NCUT_TABLE) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) image_sum<0, O2>(rz[r], q[r], hi[r], hj, soft_hi[r], k, ncut_rt, S[r], T[r]);
+        return;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        double w0 = inv_cube_sqrt(q[r]);
+        if (hi32(q[r]) <= soft_hi[r]) {
+            const double hh = hi[r] + hj;
+            if (q[r] < hh * hh) w0 = spline_w(q[r], hh);
+        }
+        S[r] = w0;
+        T[r] = 0.0;
+    }
+#pragma unroll kRtUnroll
+    for (int n = 1; n < ncut_rt; ++n) {
+        const double c = k.c2nL[n], b = k.n2L2[n], d = k.dn[n];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double B  = q[r] + b;
+            const double wp = inv_cube_sqrt_far<O2>(fma(-c, rz[r], B));
+            const double wm = inv_cube_sqrt_far<O2>(fma(c, rz[r], B));
+            S[r] += wp;
+            S[r] += wm;
+            T[r] = fma(d, wp - wm, T[r]);
+        }
+    }
+    const double ce = k.c2nL[ncut_rt], be = k.n2L2[ncut_rt], de = k.dn[ncut_rt];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const bool rz_nonzero = ((hi32(rz[r]) & 0x7fffffff) | lo32(rz[r])) != 0;
+        double we = inv_cube_sqrt_far<O2>(fma(-ce, fabs(rz[r]), q[r] + be));
+        we = rz_nonzero ? we : 0.0;
+        S[r] += we;
+        T[r] = fma(copysign(de, rz[r]), we, T[r]);
     }
 }
 

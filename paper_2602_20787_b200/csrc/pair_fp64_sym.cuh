@@ -65,6 +65,34 @@ __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&
         const double2 pa = *reinterpret_cast<const double2 *>(&sj->x);
         const double2 pb = *reinterpret_cast<const double2 *>(&sj->z);
         const double hj = sj->h;
+        if constexpr (NC == 0) {
+            // run-time N_cut: all R targets go through the image loop together (image_sum_rt)
+            double rx[R], ry[R], rz[R], q[R], hi[R], S[R], T[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                rx[r] = ti[r].x - pa.x;
+                ry[r] = ti[r].y - pa.y;
+                rz[r] = nearest_image(ti[r].z - pb.x, k);
+                q[r] = fma(rz[r], rz[r], fma(ry[r], ry[r], rx[r] * rx[r]));
+                hi[r] = ti[r].h;
+            }
+            image_sum_rt<R, O2>(rz, q, hi, hj, soft_hi, k, ncut_rt, S, T);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double Sj = pb.y * S[r];
+                a[r][0] = fma(Sj, rx[r], a[r][0]);
+                a[r][1] = fma(Sj, ry[r], a[r][1]);
+                a[r][2] = fma(Sj, rz[r], a[r][2]);
+                a[r][3] = fma(pb.y, T[r], a[r][3]);
+                if (SYM) {
+                    const double Si = ti[r].m * S[r];
+                    bx = fma(Si, rx[r], bx);
+                    by = fma(Si, ry[r], by);
+                    bz = fma(Si, rz[r], bz);
+                    bz = fma(ti[r].mL, T[r], bz);
+                }
+            }
+        } else
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;

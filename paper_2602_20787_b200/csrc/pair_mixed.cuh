@@ -18,10 +18,17 @@
 
 namespace steps {
 
+#ifndef STEPS_RT_UNROLL_MIXED
+#define STEPS_RT_UNROLL_MIXED 3
+#endif
+constexpr int kRtUnrollMixed = STEPS_RT_UNROLL_MIXED;   // run-time N_cut image loop of the packed mixed kernel
+                                                        // (1/2/3/4 at N_cut = 10: 237 / 223 / 214 / 215 ms)
+
 struct MixedConsts {
     float Lh, Ll, halfL;
-    float c2nL[MAX_NCUT_UNROLLED + 1];
-    float n2L2[MAX_NCUT_UNROLLED + 1];
+    float c2nL[MAX_NCUT_TABLE + 1];       // 2 n L
+    float n2L2[MAX_NCUT_TABLE + 1];       // (n L)^2
+    float dn[MAX_NCUT_TABLE + 1];         // n
 };
 
 __device__ __forceinline__ float rsqrt_f32(float x)
@@ -88,6 +95,21 @@ __device__ __forceinline__ void pair_term_mixed(const float4 &ih, const float4 &
         we = (rz == 0.0f) ? 0.0f : we;
         S += we;
         T = fmaf(copysignf((float)NC, rz), we, T);
+    } else if (ncut_rt <= MAX_NCUT_TABLE) {
+        // run-time N_cut: per-image constants indexed out of the kernel-parameter bank
+#pragma unroll 2
+        for (int n = 1; n < ncut_rt; ++n) {
+            const float B  = q + k.n2L2[n];
+            const float wp = inv_cube_sqrt_f32(fmaf(-k.c2nL[n], rz, B));
+            const float wm = inv_cube_sqrt_f32(fmaf(k.c2nL[n], rz, B));
+            S += wp;
+            S += wm;
+            T = fmaf(k.dn[n], wp - wm, T);
+        }
+        float we = inv_cube_sqrt_f32(fmaf(-k.c2nL[ncut_rt], fabsf(rz), q + k.n2L2[ncut_rt]));
+        we = (rz == 0.0f) ? 0.0f : we;
+        S += we;
+        T = fmaf(copysignf(k.dn[ncut_rt], rz), we, T);
     } else {
         const float L = k.Lh;
         for (int n = 1; n < ncut_rt; ++n) {

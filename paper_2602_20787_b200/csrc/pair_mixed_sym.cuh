@@ -45,6 +45,21 @@ __device__ __forceinline__ void image_sum_f32(float rz, float q, float hi, float
         we = (rz == 0.0f) ? 0.0f : we;
         S += we;
         T = (NC == 1) ? copysignf(we, rz) : fmaf(copysignf((float)NC, rz), we, T);
+    } else if (ncut_rt <= MAX_NCUT_TABLE) {
+        // run-time N_cut: per-image constants indexed out of the kernel-parameter bank
+#pragma unroll 2
+        for (int n = 1; n < ncut_rt; ++n) {
+            const float B  = q + k.n2L2[n];
+            const float wp = inv_cube_sqrt_f32(fmaf(-k.c2nL[n], rz, B));
+            const float wm = inv_cube_sqrt_f32(fmaf(k.c2nL[n], rz, B));
+            S += wp;
+            S += wm;
+            T = fmaf(k.dn[n], wp - wm, T);
+        }
+        float we = inv_cube_sqrt_f32(fmaf(-k.c2nL[ncut_rt], fabsf(rz), q + k.n2L2[ncut_rt]));
+        we = (rz == 0.0f) ? 0.0f : we;
+        S += we;
+        T = fmaf(copysignf(k.dn[ncut_rt], rz), we, T);
     } else {
         const float L = k.Lh;
         for (int n = 1; n < ncut_rt; ++n) {
@@ -205,6 +220,15 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
                 S = add2(add2(S, wp), wm);
                 T = (n == 1) ? sub2(wp, wm) : fma2(bc((float)n), sub2(wp, wm), T);
             }
+        } else if (ncut_rt <= MAX_NCUT_TABLE) {
+#pragma unroll kRtUnrollMixed
+            for (int n = 1; n < ncut_rt; ++n) {
+                const float2 B  = add2(q, bc(k.n2L2[n]));
+                const float2 wp = cube2(rsqrt2(fma2(bc(-k.c2nL[n]), rz, B)));
+                const float2 wm = cube2(rsqrt2(fma2(bc(k.c2nL[n]), rz, B)));
+                S = add2(add2(S, wp), wm);
+                T = fma2(bc(k.dn[n]), sub2(wp, wm), T);
+            }
         } else {
             for (int n = 1; n < ncut_rt; ++n) {
                 const float nL = (float)n * k.Lh;
@@ -216,10 +240,11 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
             }
         }
         {   // end image n = sign(rz) N_cut, absent when rz == 0
+            const bool tab = NC > 0 || n_img <= MAX_NCUT_TABLE;         // constants from MixedConsts
             const float NL = (float)n_img * k.Lh;
             const float2 arz = make_float2(fabsf(rz.x), fabsf(rz.y));
-            const float2 Be = (NC > 0) ? add2(q, bc(k.n2L2[NC > 0 ? NC : 0])) : fma2(bc(NL), bc(NL), q);
-            float2 we = cube2(rsqrt2(fma2(bc(-2.0f * NL), arz, Be)));
+            const float2 Be = tab ? add2(q, bc(k.n2L2[tab ? n_img : 0])) : fma2(bc(NL), bc(NL), q);
+            float2 we = cube2(rsqrt2(fma2(bc(tab ? -k.c2nL[tab ? n_img : 0] : -2.0f * NL), arz, Be)));
             we.x = (rz.x == 0.0f) ? 0.0f : we.x;
             we.y = (rz.y == 0.0f) ? 0.0f : we.y;
             S = add2(S, we);

@@ -434,12 +434,14 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->mc.Lh = (float)L;
     ctx->mc.Ll = (float)(L - (double)ctx->mc.Lh);
     ctx->mc.halfL = (float)(0.5 * L);
-    for (int n = 0; n <= MAX_NCUT_UNROLLED; ++n) {
+    for (int n = 0; n <= MAX_NCUT_TABLE; ++n) {
         const double nL = (double)n * L;
         ctx->kc.c2nL[n] = 2.0 * nL;
         ctx->kc.n2L2[n] = nL * nL;
+        ctx->kc.dn[n] = (double)n;
         ctx->mc.c2nL[n] = (float)(2.0 * nL);
         ctx->mc.n2L2[n] = (float)(nL * nL);
+        ctx->mc.dn[n] = (float)n;
     }
 
     auto A = [&](cudaError_t e) { if (e != cudaSuccess && rc == STEPS_OK) { rc = (e == cudaErrorMemoryAllocation) ? STEPS_ENOMEM : STEPS_ECUDA; cuda_fail(ctx, e); } };

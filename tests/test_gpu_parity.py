@@ -86,14 +86,21 @@ def test_ragged_sizes(torch_cuda, oracle, n):
             check(g, ref, precision)
 
 
-@pytest.mark.parametrize("n_cut", [1, 2, 3, 4, 5, 6, 7, 8, 9, 12, 40])
+@pytest.mark.parametrize("n_cut", [1, 2, 3, 4, 5, 6, 7, 8, 9, 12, 40, 64, 65])
 def test_n_cut_unrolled_and_runtime_loops(torch_cuda, oracle, n_cut):
+    """N_cut <= 8: unrolled instances; 9 .. 64: run-time loop with tabulated per-image constants;
+    above: run-time loop that forms them.  Every kernel family (atomic, rounds, ordered)."""
+    from paper_2602_20787_b200 import binding as b
     from paper_2602_20787_b200 import workloads
     w = workloads.make(1, n=1500, seed=5)
     ref = oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, n_cut)
     for precision in (0, 1):
         g = gpu_accel(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, n_cut, precision)
         check(g, ref, precision)
+        if n_cut > 8:
+            for flag in (b.FLAG_DETERMINISTIC, b.FLAG_ORDERED_PAIRS):
+                g = gpu_accel(torch_cuda, (w.x, w.y, w.z, w.m, w.h), w.Lz, w.G, n_cut, precision, flags=flag)
+                check(g, ref, precision)
 
 
 @pytest.mark.parametrize("precision", [0, 1])
