@@ -92,7 +92,9 @@ typedef struct {
     double  Lz;             /* period along z, > 0                                      */
     double  G;              /* gravitational constant, any sign (G < 0: glass making)   */
     int32_t periodic_mode;  /* STEPS_PERIODIC_*                                                       */
-    int32_t n_cut;          /* N_cut of Eq. 8, >= 1: 2*N_cut images per pair                          */
+    int32_t n_cut;          /* N_cut of Eq. 8, >= 1: 2*N_cut images per pair.  Any value is accepted and gives
+                               the same sum; 1..8 run fully unrolled kernel instances, 9..64 a run-time image loop
+                               with tabulated per-image constants, larger values a loop that forms them          */
     int32_t precision;      /* STEPS_PREC_*                                                           */
     int32_t background;     /* STEPS_BG_*                                                             */
     double  R_sim;          /* radius R of the simulation volume in Eq. 9; needed if rho0 != 0 and
