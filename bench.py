@@ -31,64 +31,31 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# Instruction mix of the pair kernels' inner loops at N_cut = 5 (10 image terms per pair), counted
-# in the SASS of the shipped library (cuobjdump -sass).  "unit" says what one
-# loop iteration covers: the symmetric kernel evaluates an UNORDERED pair (two interactions).
-KERNEL_MIX = {
-    # default fp64 kernel, pair_fp64_sym_kernel<5>: one unordered pair per iteration
-    "fp64": dict(kernel="pair_fp64_sym_kernel<5>", interactions=2, dfma=53, dmul=33, dadd=22, dsetp=0,
-                 per_image=(9.5, 14.0)),
-    # STEPS_FLAG_DETERMINISTIC, pair_fp64_round_kernel<5>: the same loop, scheduled in conflict-free rounds
-    "fp64_det": dict(kernel="pair_fp64_round_kernel<5>", interactions=2, dfma=53, dmul=33, dadd=22, dsetp=0,
-                     per_image=(9.5, 14.0)),
-    # STEPS_FLAG_ORDERED_PAIRS, pair_fp64_kernel<5,0>: one ordered pair per iteration
-    "fp64_ord": dict(kernel="pair_fp64_kernel<5,0>", interactions=1, dfma=49, dmul=32, dadd=22, dsetp=0,
-                     per_image=(9.5, 14.0)),
-    # --periodic table: pair_table_sym_kernel<CIC, 4, false> (softened nearest image + 4 gathers of double2
-    # nodes through L1), one unordered pair per iteration; independent of n_cut
-    "table": dict(kernel="pair_table_sym_kernel<CIC>", interactions=2, dfma=23, dmul=13, dadd=17, dsetp=4,
-                  per_image=(0.0, 0.0)),
-    # --periodic table --table-fp32: pair_table_sym_kernel<CIC, 16, true> (float nodes in shared memory,
-    # their weighted sum in fp32: 8 FADD + 6 FFMA per pair, not counted as FP64 work)
-    "table_f32": dict(kernel="pair_table_sym_kernel<CIC,fp32 nodes>", interactions=2, dfma=17, dmul=13, dadd=11,
-                      dsetp=3, per_image=(0.0, 0.0)),
-    # --periodic table --precision mixed: pair_table_mixed_sym_kernel<CIC>, one unordered pair per iteration
-    "mixed_table": dict(kernel="pair_table_mixed_sym_kernel<CIC>", interactions=2, ffma=19, fmul=10, fadd=23,
-                        mufu=2, f2f=0, dadd=0),
-    # default mixed kernel, pair_mixed_sym_kernel<5>: one unordered pair per iteration (FP32-pipe
-    # instructions + 10 MUFU.RSQ; conversions and DADDs are outside the per-pair loop)
-    # (main loop: 38 FFMA2 + 19 FMUL2 + 16 FADD2 + 20 MUFU per ring step of two unordered pairs; counted
-    # here as scalar FP32 operations per unordered pair)
-    "mixed": dict(kernel="pair_mixed_sym_kernel<5>", interactions=2, ffma=38, fmul=19, fadd=16, mufu=10,
-                  f2f=0, dadd=0),
-    # STEPS_FLAG_DETERMINISTIC, pair_mixed_round_kernel<5>: the same loop in conflict-free rounds
-    "mixed_det": dict(kernel="pair_mixed_round_kernel<5>", interactions=2, ffma=38, fmul=19, fadd=16, mufu=10,
-                      f2f=0, dadd=0),
-    # STEPS_FLAG_ORDERED_PAIRS, pair_mixed_kernel<5>: one ordered pair per iteration
-    "mixed_ord": dict(kernel="pair_mixed_kernel<5>", interactions=1, ffma=17, fmul=27, fadd=30, mufu=10,
-                      f2f=4, dadd=4),
-}
 METRIC = "pair interactions/s (N=1M, periodic-z, fp64); % of B200 FP64 FMA peak"
 NOMINAL_FP64_LANES_PER_SM = 64
 NOMINAL_FP32_LANES_PER_SM = 128
 NOMINAL_XU_LANES_PER_SM = 16
-NCU_DRAM_BYTES_DEFAULT = 78.49e6 + 8.60e6     # pair_fp64_sym_kernel<5>, N = 1 048 576 (algorithmic: 42 MB + 34 MB)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_dram_traffic.csv")
 
 
-def pipe_counts(mode, n_cut):
-    """(pipe instructions, flops) per ORDERED pair interaction for the kernel of `mode`."""
-    mix = KERNEL_MIX[mode]
-    if mode.startswith("mixed"):
-        instr = mix["ffma"] + mix["fmul"] + mix["fadd"]
-        flops = 2 * mix["ffma"] + mix["fmul"] + mix["fadd"]
-        d = 0 if mode == "mixed_table" else 2 * (n_cut - 5)
-        return (instr + 7.5 * d) / mix["interactions"], (flops + 9.0 * d) / mix["interactions"]
-    instr = mix["dfma"] + mix["dmul"] + mix["dadd"] + mix["dsetp"]
-    flops = 2 * mix["dfma"] + mix["dmul"] + mix["dadd"]
-    d = 0 if mode.startswith("table") else 2 * (n_cut - 5)   # extra image terms per pair evaluation
-    instr += mix["per_image"][0] * d
-    flops += mix["per_image"][1] * d
-    return instr / mix["interactions"], flops / mix["interactions"]
+def pipe_counts(kernel, n_cut):
+    """Pipe instructions / flops per ORDERED pair interaction of `kernel`, from the SASS tally build.py wrote
+    beside the library (paper_2602_20787_b200/sassmix.py); never a literal in this file."""
+    from paper_2602_20787_b200 import build, sassmix
+    return sassmix.per_interaction(sassmix.load(build.SASSMIX), kernel, n_cut)
+
+
+def ncu_traffic(kernel, n, n_cut):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` at (n, n_cut), from the committed
+    `ncu --set full` rows in profiles/ncu_dram_traffic.csv (None if that configuration was never captured)."""
+    import csv
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, None
+    with open(TRAFFIC_CSV) as f:
+        for row in csv.DictReader(l for l in f if not l.startswith("#")):
+            if row["kernel"] == kernel and int(row["n"]) == n and int(row["n_cut"]) in (n_cut, -1):
+                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), row["source"]
+    return None, None
 
 
 class ClockSampler:
@@ -229,6 +196,51 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def make_ctx(b, w, local, args, precision, periodic, tab_fp32, interp, flags):
+    table = periodic == "table"
+    # table mode sums all images (N_cut -> inf), so its consistent background term is Eq. 10
+    return b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=args.n_cut,
+                      precision=b.PREC_MIXED if precision == "mixed" else b.PREC_FP64,
+                      background=b.BG_INFINITE if table else b.BG_FINITE,
+                      R_sim=w.R_sim, rho0=w.rho0, device=local,
+                      periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
+                      tab_fp32=1 if (table and tab_fp32) else 0,
+                      interp=b.INTERP_TSC if (table and interp == "tsc") else b.INTERP_CIC, flags=flags)
+
+
+def roofline_of(ctx, n, n_cut, t_pair, sm_count, sm_max, table):
+    """Roofline record of the all-pairs kernel `ctx` launches: numerator from the SASS tally of the built
+    library, duration from the CUDA events the library records around that launch."""
+    kernel = ctx.pair_kernel_name()
+    cnt, how = pipe_counts(kernel, n_cut)
+    pairs = float(n) * float(n - 1)
+    is_mixed = "mixed" in kernel
+    lanes = NOMINAL_FP32_LANES_PER_SM if is_mixed else NOMINAL_FP64_LANES_PER_SM
+    instr = cnt["fp32_ops"] if is_mixed else cnt["fp64_instr"]
+    flops = cnt["fp32_flops"] if is_mixed else cnt["fp64_flops"]
+    nominal_tflops = sm_count * lanes * 2 * sm_max * 1e6 / 1e12
+    achieved_tflops = flops * pairs / t_pair / 1e12
+    traffic, traffic_src = ncu_traffic(kernel, n, -1 if table else n_cut)
+    r = {
+        "bound": "alu", "kernel": kernel, "achieved": achieved_tflops, "peak": nominal_tflops,
+        "unit": "TFLOP/s", "frac": achieved_tflops / nominal_tflops,
+        "traffic": traffic, "traffic_source": traffic_src,
+        "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum); the bound is the "
+                        "%s pipe, not HBM" % ("FP32" if is_mixed else "FP64"),
+        "algorithmic_bytes": 72.0 * n,
+        "peak_kind": "nominal %s FMA: %d SMs x %d lanes x 2 flop x %.0f MHz (DESIGN.md)"
+                     % ("FP32" if is_mixed else "FP64", sm_count, lanes, sm_max),
+        "counting": "SASS tally of the built library (sassmix.py, %s); FMA = 2 flop, ADD/MUL = 1" % how,
+        "flops_per_pair_interaction": flops, "pipe_instr_per_pair_interaction": instr,
+        "pipe_util_vs_nominal": instr * pairs / t_pair / (nominal_tflops * 1e12 / 2),
+        "kernel_ms": 1e3 * t_pair,
+    }
+    if is_mixed or cnt["fp32_ops"] > 0:
+        xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
+        r["xu_pipe_util_vs_nominal"] = (cnt["mufu"] + cnt["conv"]) * pairs / t_pair / xu_peak
+    return r
+
+
 def run_ours(args):
     import torch
     from paper_2602_20787_b200 import binding as b
@@ -250,125 +262,115 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    prec = b.PREC_MIXED if args.precision == "mixed" else b.PREC_FP64
     # replicas only: every rank integrates its own particle set
     w = workloads.make(3, n=args.n, seed=3 + rank)
     n = w.n
     table = args.periodic == "table"
-    # table mode sums all images (N_cut -> inf), so its consistent background term is Eq. 10
-    ctx = b.StepsCyl(n=n, Lz=w.Lz, G=w.G, n_cut=args.n_cut, precision=prec,
-                     background=b.BG_INFINITE if table else b.BG_FINITE,
-                     R_sim=w.R_sim, rho0=w.rho0, device=local,
-                     periodic_mode=b.PERIODIC_EWALD_TABLE if table else b.PERIODIC_IMAGES,
-                     tab_fp32=1 if (table and args.table_fp32) else 0,
-                     interp=b.INTERP_TSC if (table and args.interp == "tsc") else b.INTERP_CIC,
-                     flags=(b.FLAG_DETERMINISTIC if args.deterministic else 0)
-                     | (b.FLAG_ORDERED_PAIRS if args.ordered else 0)
-                     | (b.FLAG_FAR_ORDER2 if args.far_order2 else 0))
+    flags = ((b.FLAG_DETERMINISTIC if args.deterministic else 0) | (b.FLAG_ORDERED_PAIRS if args.ordered else 0)
+             | (b.FLAG_FAR_ORDER2 if args.far_order2 else 0) | (b.FLAG_GRAPH if args.graph else 0))
     names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
-    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).pin_memory()
-            for k in names}
-    dev = {k: host[k].cuda(non_blocking=True) for k in names}
-    g = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
-    ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)       # g(x_0), untimed
-    ctx.check()
-    hg = [t.cpu().pin_memory() for t in g]
-    dfma_per_s = ctx.fp64_peak(200.0)
-    sched = cosmo_schedule(w, 2 * (args.warmup + args.steps) + 2)
+    host0 = {k: np.ascontiguousarray(getattr(w, k), dtype=np.float64) for k in names}
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-
-    def step(k):
-        flush.zero_()
-        ctx.kdk_step(*[dev[q] for q in names], *g, *sched[k], w.cosmo["dt"])
-
-    launches0 = ctx.launch_count()
-    for k in range(args.warmup):
-        step(k)
-    launches_per_step = (ctx.launch_count() - launches0) / max(args.warmup, 1)
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    pair_ms = []
-    ev[0].record()
-    for k in range(args.steps):
-        step(args.warmup + k)
-        pair_ms.append(ctx.last_pair_kernel_ms())          # waits for that launch's end event
-    ev[1].record()
-    barrier()
-    clocks = sampler.stop() if rank == 0 else {}
-    ctx.check()
-    t_dev = max_over_ranks(ev[0].elapsed_time(ev[1]) * 1e-3, dist, "cuda")
     pairs_per_step = float(n) * float(n - 1)
-    value = replica_throughput(pairs_per_step, args.steps, world, t_dev)
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    peaks, peaks_kind = load_peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
 
-    # end to end: pinned host buffers through steps_cyl_kdk_step_host, copies inside the timing
-    hs = [host[q] for q in names] + hg
-    for k in range(1):
-        ctx.kdk_step_host(*hs, *sched[args.warmup + args.steps + k], w.cosmo["dt"])
-    barrier()
-    t0 = time.perf_counter()
-    for k in range(args.steps):
-        ctx.kdk_step_host(*hs, *sched[args.warmup + args.steps + 1 + k], w.cosmo["dt"])
-    torch.cuda.synchronize()
-    e2e_value = replica_throughput(pairs_per_step, args.steps, world,
-                                   max_over_ranks(time.perf_counter() - t0, dist, "cuda"))
-    assert all(bool(torch.isfinite(t).all()) for t in hg)
+    def measure(precision, periodic, tab_fp32, interp, flags, steps, warmup, e2e_steps, sample_clocks):
+        """One mode: fresh context and particle state; W warm-up + K timed KDK steps (device time, L2 flushed
+        between steps), then the same step through the host-pointer entry point."""
+        ctx = make_ctx(b, w, local, args, precision, periodic, tab_fp32, interp, flags)
+        host = {k: torch.from_numpy(host0[k].copy()).pin_memory() for k in names}
+        dev = {k: host[k].cuda(non_blocking=True) for k in names}
+        g = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)       # g(x_0), untimed
+        ctx.check()
+        hg = [t.cpu().pin_memory() for t in g]
+        sched = cosmo_schedule(w, warmup + steps + e2e_steps + 2)
+
+        def step(k):
+            flush.zero_()
+            ctx.kdk_step(*[dev[q] for q in names], *g, *sched[k], w.cosmo["dt"])
+
+        launches0 = ctx.launch_count()
+        for k in range(warmup):
+            step(k)
+        launches_per_step = (ctx.launch_count() - launches0) / max(warmup, 1)
+        barrier()
+        sampler = ClockSampler(local)
+        if rank == 0 and sample_clocks:
+            sampler.start()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        pair_ms = []
+        ev[0].record()
+        for k in range(steps):
+            step(warmup + k)
+            pair_ms.append(ctx.last_pair_kernel_ms())          # waits for that launch's end event
+        ev[1].record()
+        barrier()
+        clocks = sampler.stop() if (rank == 0 and sample_clocks) else {}
+        ctx.check()
+        t_dev = max_over_ranks(ev[0].elapsed_time(ev[1]) * 1e-3, dist, "cuda")
+        out = {"ctx": ctx, "t_dev": t_dev, "t_pair": float(np.mean(pair_ms)) * 1e-3, "clocks": clocks,
+               "launches_per_step": launches_per_step, "value": replica_throughput(pairs_per_step, steps, world, t_dev),
+               "e2e_value": None}
+        if e2e_steps:
+            # end to end: pinned host buffers through steps_cyl_kdk_step_host, copies inside the timing
+            hs = [host[q] for q in names] + hg
+            ctx.kdk_step_host(*hs, *sched[warmup + steps], w.cosmo["dt"])
+            barrier()
+            t0 = time.perf_counter()
+            for k in range(e2e_steps):
+                ctx.kdk_step_host(*hs, *sched[warmup + steps + 1 + k], w.cosmo["dt"])
+            torch.cuda.synchronize()
+            out["e2e_value"] = replica_throughput(pairs_per_step, e2e_steps, world,
+                                                  max_over_ranks(time.perf_counter() - t0, dist, "cuda"))
+            assert all(bool(torch.isfinite(t).all()) for t in hg)
+        return out
+
+    main = measure(args.precision, args.periodic, args.table_fp32, args.interp, flags, args.steps, args.warmup,
+                   args.steps, True)
+    ctx = main["ctx"]
+    dfma_per_s = ctx.fp64_peak(200.0) if rank == 0 else 0.0
+
+    # the other modes north_star names, in the same run (rank 0's line carries them; all ranks run them so that the
+    # barriers match): mixed precision against the FP32 peak, and the Ewald-table mode of Eq. 12-17
+    subs = {}
+    default_line = (args.precision == "fp64" and not table and flags == 0)
+    if default_line and not args.no_sub:
+        k_sub, w_sub = min(args.steps, 3), 3
+        for key, (prec, per, f32) in (("mixed", ("mixed", "images", False)),
+                                      ("table", ("fp64", "table", False)),
+                                      ("table_fp32", ("fp64", "table", True)),
+                                      ("table_mixed", ("mixed", "table", True))):
+            subs[key] = measure(prec, per, f32, "cic", 0, k_sub, w_sub, 0, True)
+            subs[key]["steps"], subs[key]["warmup"] = k_sub, w_sub
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    peaks, peaks_kind = load_peaks()
-    if table:
-        mode = "mixed_table" if prec == b.PREC_MIXED else ("table_f32" if args.table_fp32 else "table")
-    else:
-        mode = ("mixed" if prec == b.PREC_MIXED else "fp64") + ("_det" if args.deterministic else "")
-        if args.ordered:
-            mode = "mixed_ord" if prec == b.PREC_MIXED else "fp64_ord"
-    instr, flops = pipe_counts(mode, args.n_cut)
-    if args.far_order2 and mode == "fp64":              # one DFMA less per far image
-        instr -= (2 * args.n_cut - 1) / 2.0
-        flops -= (2 * args.n_cut - 1)
-    t_pair = float(np.mean(pair_ms)) * 1e-3
-    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    is_mixed = mode.startswith("mixed")
-    lanes = NOMINAL_FP32_LANES_PER_SM if is_mixed else NOMINAL_FP64_LANES_PER_SM
-    nominal_tflops = sm_count * lanes * 2 * sm_max * 1e6 / 1e12
-    achieved_tflops = flops * pairs_per_step / t_pair / 1e12
-    roofline = {
-        "bound": "alu", "kernel": KERNEL_MIX[mode]["kernel"].replace("<5", "<%d" % args.n_cut),
-        "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
-        "frac": achieved_tflops / nominal_tflops,
-        # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one `ncu --set full` capture of the
-        # default configuration (profiles/r1_ncu_full_pair_kernels.md); other configurations: not captured
-        "traffic": NCU_DRAM_BYTES_DEFAULT if (mode == "fp64" and n == 1048576 and args.n_cut == 5) else None,
-        "traffic_unit": "bytes per launch (ncu); the bound is the FP64 pipe, not HBM",
-        "peak_kind": "nominal %s FMA: %d SMs x %d lanes x 2 flop x %.0f MHz (DESIGN.md)"
-                     % ("FP32" if is_mixed else "FP64", sm_count, lanes, sm_max),
-        "flops_per_pair_interaction": flops, "pipe_instr_per_pair_interaction": instr,
-        "pipe_util_vs_nominal": instr * pairs_per_step / t_pair / (nominal_tflops * 1e12 / 2),
-        "kernel_ms": 1e3 * t_pair, "kernel_share_of_step": t_pair * args.steps / t_dev,
-    }
-    if table and args.deterministic:                       # same loops, scheduled in rounds (pair_table_round.cuh)
-        roofline["kernel"] = roofline["kernel"].replace("sym_kernel", "round_kernel")
-    if table and args.interp == "tsc":
-        # the instruction tallies above are those of the CIC loops; the TSC loops (9 gathers) are not tallied
-        roofline["kernel"] = roofline["kernel"].replace("CIC", "TSC")
-        for key in ("achieved", "frac", "flops_per_pair_interaction", "pipe_instr_per_pair_interaction",
-                    "pipe_util_vs_nominal"):
-            roofline[key] = None
-    if is_mixed:
-        xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
-        mufu = ((KERNEL_MIX[mode]["mufu"] if table else 2 * args.n_cut) + KERNEL_MIX[mode]["f2f"]) \
-            / KERNEL_MIX[mode]["interactions"]
-        roofline["xu_pipe_util_vs_nominal"] = mufu * pairs_per_step / t_pair / xu_peak
-    else:
+    t_dev, t_pair = main["t_dev"], main["t_pair"]
+    roofline = roofline_of(ctx, n, args.n_cut, t_pair, sm_count, sm_max, table)
+    roofline["kernel_share_of_step"] = t_pair * args.steps / t_dev
+    if "mixed" not in roofline["kernel"]:
         roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
-        roofline["pipe_util_vs_measured_dfma"] = (None if roofline["frac"] is None
-                                                  else instr * pairs_per_step / t_pair / dfma_per_s)
+        roofline["pipe_util_vs_measured_dfma"] = (roofline["pipe_instr_per_pair_interaction"] * pairs_per_step
+                                                  / t_pair / dfma_per_s)
+    sub_records = {}
+    for key, m in subs.items():
+        is_tab = key.startswith("table")
+        r = roofline_of(m["ctx"], n, args.n_cut, m["t_pair"], sm_count, sm_max, is_tab)
+        sub_records[key] = {
+            "value": m["value"], "unit": "pairs/s", "steps": m["steps"], "warmup": m["warmup"],
+            "ms_per_step": 1e3 * m["t_dev"] / m["steps"], "seconds_per_force_evaluation": m["t_pair"],
+            "dtype": {"mixed": "f32 pair terms, f64 accumulation", "table": "f64",
+                      "table_fp32": "f64 pair terms, f32 table nodes and interpolation",
+                      "table_mixed": "f32 pair terms and table, f64 accumulation"}[key],
+            "periodic": "Ewald table 144x128 CIC, rho_max=5L, all images (Eq. 12-17)" if is_tab
+                        else "n_cut=%d (%d images/pair)" % (args.n_cut, 2 * args.n_cut),
+            "roofline": r, "clocks": m["clocks"], "gpu_launches": int(round(m["launches_per_step"] * m["steps"])),
+        }
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -379,27 +381,33 @@ def run_ours(args):
         cpu = {"value": len(idx) * (n - 1) / tc, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                "sample": "oracle.accel on %d seeded targets x all %d sources (force evaluation only), "
                          "%.1f s" % (len(idx), n, tc)}
+    mixed_prec = args.precision == "mixed"
     periodic_desc = ("Ewald table 144x128 %s%s, (n_max,m_max)=(5,12), rho_max=5L, background Eq. 10"
-                     % (args.interp.upper(), " (float nodes in shared memory)" if (args.table_fp32 or prec == b.PREC_MIXED) else "") if table
+                     % (args.interp.upper(), " (float nodes in shared memory)" if (args.table_fp32 or mixed_prec) else "") if table
                      else "n_cut=%d (%d images/pair), background Eq. 9" % (args.n_cut, 2 * args.n_cut))
+    if mixed_prec:
+        dtype = "f32"            # pair terms in float (hi/lo separations), accumulation in double
+    elif table and args.table_fp32:
+        dtype = "f64+f32"        # pair terms in double, table nodes and their interpolation in float
+    else:
+        dtype = "f64"
     line = {
-        "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": main["value"], "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64" if prec == b.PREC_FP64 else "f32",
-        "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving KDK step (Om=0.3, OL=0.7, "
                                "a 0.02->0.025), L=100 Mpc/h, r_max=1000, %s" % (n, periodic_desc),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB buffer written between steps (L2 flush)"},
-        "image_terms_per_s": None if table else value * 2 * args.n_cut,
+        "image_terms_per_s": None if table else main["value"] * 2 * args.n_cut,
         "seconds_per_force_evaluation": t_pair,
-        "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": 11 * 8 * n,
+        "roofline": roofline, "cpu_baseline": cpu, "clocks": main["clocks"],
+        "e2e": {"value": main["e2e_value"], "unit": "pairs/s", "h2d_bytes_per_step": 11 * 8 * n,
                 "d2h_bytes_per_step": 9 * 8 * n},
-        "gpu_launches": int(round(launches_per_step * args.steps)),
+        "gpu_launches": int(round(main["launches_per_step"] * args.steps)),
         "peaks_file": peaks_kind,
     }
+    line.update(sub_records)          # "mixed", "table", "table_fp32", "table_mixed" (default line only)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -425,6 +433,10 @@ def main():
     ap.add_argument("--table-fp32", action="store_true",
                     help="--periodic table: float table held in shared memory (tab_fp32 = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sub", action="store_true",
+                    help="default line only: skip the mixed / table sub-records measured in the same run")
+    ap.add_argument("--graph", action="store_true",
+                    help="STEPS_FLAG_GRAPH: the KDK step replayed as one captured CUDA graph")
     ap.add_argument("--deterministic", action="store_true",
                     help="STEPS_FLAG_DETERMINISTIC: bit-reproducible (fp64: round-scheduled symmetric kernel)")
     ap.add_argument("--ordered", action="store_true",

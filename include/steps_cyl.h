@@ -39,6 +39,8 @@
  *   - z may lie outside [0, Lz): it is reduced to [0, Lz) first (periodicity).
  *     NaN / Inf inputs are not checked (garbage in, garbage out).
  *   - There is NO CPU fallback: without a CUDA device steps_cyl_init returns STEPS_ECUDA.
+ *   - Every call that takes a context makes params.device current while it runs and restores the
+ *     caller's current device before it returns.
  */
 #ifndef STEPS_CYL_H
 #define STEPS_CYL_H
@@ -83,12 +85,17 @@ enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default
                                           sums over all its sources (ordered pairs, fixed-order reduction,
                                           bit-reproducible, ~1.9x slower than the default)             */ };
 
+/* Largest particle number one context takes: the symmetric kernels put chunks of <= 64 source tiles of 128
+ * particles on gridDim.y (<= 65535).  (At 40 B/particle in and ~250 B/particle of scratch this is also
+ * about what 180 GB hold.) */
+#define STEPS_CYL_MAX_N ((int64_t)64 * 65535 * 128)
+
 typedef struct steps_cyl_ctx steps_cyl_ctx;   /* opaque; created by init, freed by destroy */
 
 /* Plain-old-data parameter block (the quantities the problem statement
  * names).  Zero-initialise, then fill. */
 typedef struct {
-    int64_t n;              /* number of particles, 1 <= n < 2^31                                     */
+    int64_t n;              /* number of particles, 1 <= n <= STEPS_CYL_MAX_N (else EINVAL at init)   */
     double  Lz;             /* period along z, > 0                                      */
     double  G;              /* gravitational constant, any sign (G < 0: glass making)   */
     int32_t periodic_mode;  /* STEPS_PERIODIC_*                                                       */
@@ -217,6 +224,10 @@ int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s);
 /* Milliseconds the device spent in the most recent all-pairs kernel launch of this context
  * (CUDA events recorded around that launch on its stream); synchronises on the end event. */
 int steps_cyl_last_pair_kernel_ms(steps_cyl_ctx *ctx, float *ms);
+
+/* Name of the all-pairs kernel this context launches for its parameters, as the SASS tally
+ * (paper_2602_20787_b200/sassmix.py) spells it, e.g. "pair_fp64_sym_kernel<5,false>".  Static per context. */
+const char *steps_cyl_pair_kernel_name(steps_cyl_ctx *ctx);
 
 const char *steps_cyl_strerror(int code);
 const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx);

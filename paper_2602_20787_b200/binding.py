@@ -25,7 +25,8 @@ EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_
            "steps_cyl_check", "steps_cyl_background", "steps_cyl_kdk_step",
            "steps_cyl_kdk_step_host",
            "steps_cyl_friedmann_step", "steps_cyl_friedmann_step_cpl", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
-           "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count"]
+           "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count",
+           "steps_cyl_pair_kernel_name"]
 
 
 class Params(C.Structure):
@@ -87,6 +88,8 @@ def lib():
         L.steps_cyl_strerror.argtypes = [C.c_int]
         L.steps_cyl_last_cuda_error.restype = C.c_char_p
         L.steps_cyl_last_cuda_error.argtypes = [vp]
+        L.steps_cyl_pair_kernel_name.restype = C.c_char_p
+        L.steps_cyl_pair_kernel_name.argtypes = [vp]
         L.steps_cyl_launch_count.restype = i64
         L.steps_cyl_launch_count.argtypes = [vp]
         _lib = L
@@ -238,6 +241,9 @@ class StepsCyl:
         if rc:
             self._raise(rc)
         return out.value
+
+    def pair_kernel_name(self):
+        return lib().steps_cyl_pair_kernel_name(self._ctx).decode()
 
     def launch_count(self):
         return int(lib().steps_cyl_launch_count(self._ctx))

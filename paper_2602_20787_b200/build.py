@@ -15,8 +15,16 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsteps_cyl.so")
 SOURCES = [os.path.join(CSRC, "steps_cyl.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("pair_fp64.cuh", "pair_fp64_sym.cuh", "pair_mixed.cuh", "pair_mixed_sym.cuh", "pair_table_sym.cuh", "pair_table_mixed_sym.cuh", "ewald_table.h", "aux_kernels.cuh")] \
-    + [os.path.join(os.path.dirname(HERE), "include", "steps_cyl.h")]
+SASSMIX = os.path.join(HERE, "libsteps_cyl.sassmix.json")
+
+
+def _deps() -> list:
+    """Everything the library is compiled from: all of csrc/ plus the public header (content-hashed)."""
+    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h")))
+    return files + [os.path.join(os.path.dirname(HERE), "include", "steps_cyl.h"),
+                    os.path.join(HERE, "sassmix.py")]
+
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC",
               "--fmad=true", "-cudart", "static"]
@@ -36,7 +44,7 @@ def _extra() -> list:
 def _source_hash() -> str:
     import hashlib
     h = hashlib.sha256(" ".join(NVCC_FLAGS + _extra()).encode())
-    for d in DEPS:
+    for d in _deps():
         h.update(open(d, "rb").read())
     return h.hexdigest()
 
@@ -46,14 +54,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     gpurun snapshot does not preserve mtimes)."""
     stamp = LIB + ".hash"
     want = _source_hash()
-    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == want:
-        return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc(), *NVCC_FLAGS, *_extra(), *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", tmp]
-    subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
-    with open(stamp, "w") as f:
-        f.write(want + "\n")
+    fresh = os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == want
+    if force or not fresh:
+        tmp = LIB + ".tmp.%d" % os.getpid()
+        cmd = [nvcc(), *NVCC_FLAGS, *_extra(), *(["-Xptxas", "-v"] if verbose else []), *SOURCES, "-o", tmp]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, LIB)
+        if os.path.exists(SASSMIX):
+            os.unlink(SASSMIX)
+        with open(stamp, "w") as f:
+            f.write(want + "\n")
+    if not os.path.exists(SASSMIX):
+        # instruction tally of the pair loops of THIS binary (bench.py's roofline numerator)
+        from . import sassmix
+        sassmix.write(LIB, SASSMIX)
     return LIB
 
 

@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -57,6 +58,7 @@ struct steps_cyl_ctx {
     bool ev_valid = false;
     bool bg_valid = false;                         // bx/by hold b(x) for the caller's current x
     int64_t launches = 0;
+    char kernel_name[96];                          // the all-pairs kernel launch_pair() selects (sassmix.py naming)
     char cuda_msg[256];
 };
 
@@ -73,6 +75,25 @@ int cuda_fail(steps_cyl_ctx *c, cudaError_t e)
         cudaError_t e_ = (call);                                     \
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_);            \
     } while (0)
+
+// Makes the context's device current for the duration of an API call and puts the caller's back afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev)
+    {
+        int cur = -1;
+        err = cudaGetDevice(&cur);
+        if (err == cudaSuccess && cur != dev) {
+            err = cudaSetDevice(dev);
+            if (err == cudaSuccess) prev = cur;
+        }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE(ctx_)                                              \
+    DeviceGuard dev_guard_((ctx_)->p.device);                        \
+    if (dev_guard_.err != cudaSuccess) return cuda_fail((ctx_), dev_guard_.err)
 
 template <typename T>
 cudaError_t dev_alloc(T **p, size_t count)
@@ -100,6 +121,34 @@ std::vector<QuadNode> make_nodes(double R)
         v.push_back(q);
     }
     return v;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-function, process-wide setting: contexts with tables of
+// different sizes can be alive together, so the limits are only ever raised (to the largest table seen).
+cudaError_t raise_table_smem_limits(size_t fp64_bytes, size_t mixed_bytes)
+{
+    static std::mutex mu;
+    static size_t cur_fp64 = 0, cur_mixed = 0;
+    std::lock_guard<std::mutex> lock(mu);
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto *kernel, size_t bytes) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    };
+    if (fp64_bytes > cur_fp64) {
+        set(pair_table_sym_kernel<0, 16, true>, fp64_bytes);
+        set(pair_table_sym_kernel<1, 16, true>, fp64_bytes);
+        set(pair_table_round_kernel<0, 16, true>, fp64_bytes);
+        set(pair_table_round_kernel<1, 16, true>, fp64_bytes);
+        if (e == cudaSuccess) cur_fp64 = fp64_bytes;
+    }
+    if (mixed_bytes > cur_mixed) {
+        set(pair_table_mixed_sym_kernel<0>, mixed_bytes);
+        set(pair_table_mixed_sym_kernel<1>, mixed_bytes);
+        set(pair_table_mixed_round_kernel<0>, mixed_bytes);
+        set(pair_table_mixed_round_kernel<1>, mixed_bytes);
+        if (e == cudaSuccess) cur_mixed = mixed_bytes;
+    }
+    return e;
 }
 
 void choose_chunks(steps_cyl_ctx *c)
@@ -235,6 +284,29 @@ void launch_table_rounds(steps_cyl_ctx *c, cudaStream_t s)
     c->launches += last + 1;
 }
 
+// The kernel launch_pair() selects, spelled as sassmix.py spells the template instances.
+void name_pair_kernel(steps_cyl_ctx *c)
+{
+    const bool mixed = c->p.precision == STEPS_PREC_MIXED, det = c->use_rounds, ord = !c->use_sym && !c->use_rounds;
+    const int nc = c->p.n_cut <= MAX_NCUT_UNROLLED ? c->p.n_cut : 0;
+    char *o = c->kernel_name;
+    const size_t cap = sizeof c->kernel_name;
+    if (c->table_mode) {
+        const int ip = c->tc.interp == STEPS_INTERP_CIC ? 0 : 1;
+        if (mixed) snprintf(o, cap, "pair_table_mixed_%s_kernel<%d>", det ? "round" : "sym", ip);
+        else snprintf(o, cap, "pair_table_%s_kernel<%d,%s>", det ? "round" : "sym", ip, c->d_table_f32 ? "16,true" : "4,false");
+    } else if (ord) {
+        if (mixed) snprintf(o, cap, "pair_mixed_kernel<%d>", nc);
+        else snprintf(o, cap, "pair_fp64_kernel<%d,0>", nc);
+    } else if (det) {
+        snprintf(o, cap, "pair_%s_round_kernel<%d,%s>", mixed ? "mixed" : "fp64", nc, c->round_split > 1 ? "true" : "false");
+    } else if (mixed) {
+        snprintf(o, cap, "pair_mixed_sym_kernel<%d>", nc);
+    } else {
+        snprintf(o, cap, "pair_fp64_sym_kernel<%d,%s>", nc, (c->p.flags & STEPS_FLAG_FAR_ORDER2) ? "true" : "false");
+    }
+}
+
 void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
 {
     if (c->table_mode && c->use_rounds) {
@@ -359,7 +431,8 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
 {
     if (!p || !out) return STEPS_EINVAL;
     *out = nullptr;
-    if (p->n < 1 || p->n >= (int64_t)2147483647 - 2 * PAIR_THREADS) return STEPS_EINVAL;
+    // upper limit: the symmetric kernels put source chunks of <= 64 tiles on gridDim.y (<= 65535)
+    if (p->n < 1 || p->n > STEPS_CYL_MAX_N) return STEPS_EINVAL;
     if (!(p->Lz > 0.0) || !std::isfinite(p->Lz) || !std::isfinite(p->G)) return STEPS_EINVAL;
     if (p->n_cut < 1 || p->n_cut > 1000000) return STEPS_EINVAL;
     if (p->periodic_mode != STEPS_PERIODIC_IMAGES && p->periodic_mode != STEPS_PERIODIC_EWALD_TABLE)
@@ -398,7 +471,8 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device >= ndev) { delete ctx; return STEPS_ECUDA; }
-    if (cudaSetDevice(p->device) != cudaSuccess) { delete ctx; return STEPS_ECUDA; }
+    DeviceGuard dev_guard(p->device);               // the caller's current device is restored on return
+    if (dev_guard.err != cudaSuccess) { delete ctx; return STEPS_ECUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) { delete ctx; return STEPS_ECUDA; }
     ctx->sm_count = prop.multiProcessorCount;
@@ -497,14 +571,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             ctx->tcf.inv_drho = (float)((double)(pp.tab_nrho - 1) / pp.tab_rho_max);
             ctx->tcf.inv_dz = (float)((double)(pp.tab_nz - 1) / (0.5 * pp.Lz));
             ctx->tcf.two_over_L = (float)(2.0 / pp.Lz);
-            A(cudaFuncSetAttribute(pair_table_mixed_sym_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_mixed_sym_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_sym_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_sym_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_mixed_round_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_mixed_round_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_mixed_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_round_kernel<0, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
-            A(cudaFuncSetAttribute(pair_table_round_kernel<1, 16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->table_smem_bytes));
+            A(raise_table_smem_limits(ctx->table_smem_bytes, ctx->table_mixed_smem_bytes));
             if (rc != STEPS_OK) return fail(rc);
         }
         ctx->tc.D = ctx->d_table;
@@ -518,6 +585,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     }
     A(cudaMemset(ctx->flags, 0, sizeof(DevFlags)));
     if (rc != STEPS_OK) return fail(rc);
+    name_pair_kernel(ctx);
     *out = ctx;
     return STEPS_OK;
 }
@@ -539,14 +607,14 @@ int steps_cyl_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const 
                     void *cuda_stream)
 {
     if (!ctx || !x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     return enqueue_accel(ctx, x, y, z, m, h, gx, gy, gz, (cudaStream_t)cuda_stream);
 }
 
 int steps_cyl_check(steps_cyl_ctx *ctx, void *cuda_stream)
 {
     if (!ctx) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     CK(cudaStreamSynchronize((cudaStream_t)cuda_stream));
     DevFlags f;
     CK(cudaMemcpy(&f, ctx->flags, sizeof f, cudaMemcpyDeviceToHost));
@@ -558,7 +626,7 @@ int steps_cyl_accel_host(steps_cyl_ctx *ctx, const double *x, const double *y, c
                          const double *m, const double *h, double *gx, double *gy, double *gz)
 {
     if (!ctx || !x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     const size_t n = (size_t)ctx->n, B = n * sizeof(double);
     if (!ctx->host_io) {
         cudaError_t e = dev_alloc(&ctx->host_io, 11 * n);
@@ -579,7 +647,7 @@ int steps_cyl_background(steps_cyl_ctx *ctx, const double *x, const double *y, d
                          void *cuda_stream)
 {
     if (!ctx || !x || !y || !bx || !by) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     return enqueue_background(ctx, x, y, bx, by, (cudaStream_t)cuda_stream);
 }
 
@@ -590,7 +658,7 @@ int steps_cyl_kdk_step(steps_cyl_ctx *ctx, double *x, double *y, double *z, doub
 {
     if (!ctx || !x || !y || !z || !vx || !vy || !vz || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
     if (!(a_n > 0.0) || !(a_np1 > 0.0) || !std::isfinite(dt)) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const int tb = 256, nb = (ctx->n + tb - 1) / tb;
     // b(x_n): the caller may have moved the particles since the last step, so it is recomputed
@@ -617,7 +685,7 @@ int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx, double *x, double *y, double *z,
                             double H_np1, double dt)
 {
     if (!ctx || !x || !y || !z || !vx || !vy || !vz || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     const size_t n = (size_t)ctx->n, B = n * sizeof(double);
     if (!ctx->host_io) {
         cudaError_t e = dev_alloc(&ctx->host_io, 11 * n);
@@ -695,21 +763,24 @@ int steps_cyl_ewald_table(double Lz, double alpha, int32_t nmax, int32_t mmax, i
 int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s)
 {
     if (!ctx || !dfma_per_s || !(ms > 0.0)) return STEPS_EINVAL;
-    CK(cudaSetDevice(ctx->p.device));
+    ON_DEVICE(ctx);
     cudaStream_t s = ctx->own_stream;
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t err = cudaEventCreate(&e0);
+    if (err == cudaSuccess) err = cudaEventCreate(&e1);
     const int blocks = ctx->sm_count * 8, threads = 256;
     int iters = 4096;
     double best = 0.0;
-    for (int rep = 0; rep < 4; ++rep) {
-        CK(cudaEventRecord(e0, s));
-        dfma_peak_kernel<<<blocks, threads, 0, s>>>(ctx->peak_out, iters, 0.999999, 1.0e-3);
-        CK(cudaEventRecord(e1, s));
-        CK(cudaEventSynchronize(e1));
+    for (int rep = 0; rep < 4 && err == cudaSuccess; ++rep) {
         float t = 0.f;
-        CK(cudaEventElapsedTime(&t, e0, e1));
+        err = cudaEventRecord(e0, s);
+        if (err == cudaSuccess) {
+            dfma_peak_kernel<<<blocks, threads, 0, s>>>(ctx->peak_out, iters, 0.999999, 1.0e-3);
+            err = cudaEventRecord(e1, s);
+        }
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&t, e0, e1);
+        if (err != cudaSuccess) break;
         ctx->launches += 1;
         const double rate = (double)blocks * threads * 16.0 * iters / (t * 1e-3);
         if (rep > 0) best = std::max(best, rate);
@@ -717,8 +788,9 @@ int steps_cyl_fp64_peak(steps_cyl_ctx *ctx, double ms, double *dfma_per_s)
         const double scale = ms / std::max((double)t, 1e-3);
         iters = (int)std::min(4.0e6, std::max(1024.0, iters * scale));
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (err != cudaSuccess) return cuda_fail(ctx, err);
     *dfma_per_s = best;
     return STEPS_OK;
 }
@@ -745,6 +817,8 @@ const char *steps_cyl_strerror(int code)
 }
 
 const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx) { return ctx ? ctx->cuda_msg : ""; }
+
+const char *steps_cyl_pair_kernel_name(steps_cyl_ctx *ctx) { return ctx ? ctx->kernel_name : ""; }
 
 int64_t steps_cyl_launch_count(steps_cyl_ctx *ctx) { return ctx ? ctx->launches : 0; }
 

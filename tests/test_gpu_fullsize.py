@@ -1,0 +1,159 @@
+"""Full-size GPU-vs-oracle parity for BASELINE.json configs 2, 3 and 4 at their stated particle counts,
+through the C ABI, in the launch configuration bench.py times (configs 0 and 1 at full size are in
+test_gpu_parity.py).
+
+The oracle cannot evaluate N^2 pairs at these sizes, so it computes seeded SAMPLED targets one by one
+against ALL sources; properties that hold at any size (sum_i m_i g_i = 0) cover every particle.
+
+  config 2  N =   262 144  fp64, mixed, fp64 deterministic           1024 targets
+  config 3  N = 1 048 576  fp64: g at step 0, 10 KDK steps on the GPU, g at step 10 checked against
+                           the oracle evaluated on the GPU's own step-10 positions       192 targets
+                           (+ fp64 deterministic at step 0)
+  config 4  N = 4 194 304  fp64, mixed, fp64 deterministic           256 targets, half inside the spheres
+
+Bars: fp64 per-particle relative error <= 1e-10; mixed RMS <= 1e-5, max <= 1e-4 (north_star).
+STEPS_TEST_FULL_SCALE=<divisor> shrinks every N (debugging on a busy box); the driver runs it unset.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+FP64_TOL = 1e-10
+MIXED_RMS, MIXED_MAX = 1e-5, 1e-4
+SCALE = int(os.environ.get("STEPS_TEST_FULL_SCALE", "1"))
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200; there is no CPU fallback"
+    return torch
+
+
+def _targets(w, cfg, k):
+    from paper_2602_20787_b200 import workloads
+    if cfg != 4:
+        return workloads.sample_targets(w.n, k, seed=cfg)
+    # half of the targets inside the Plummer spheres (both spline branches, images near z = 0 / L)
+    ncl = w.cosmo["n_clustered"]
+    a = workloads.sample_targets(ncl, k // 2, seed=40)
+    c = ncl + workloads.sample_targets(w.n - ncl, k - k // 2, seed=41)
+    return np.sort(np.concatenate([a, c]))
+
+
+def _accel(torch, w, precision, flags):
+    from paper_2602_20787_b200 import binding as b
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda() for a in (w.x, w.y, w.z, w.m, w.h)]
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=w.n_cut, precision=precision, flags=flags)
+    try:
+        ctx.accel(*dev, *g)
+        ctx.check()
+        assert ctx.launch_count() >= 3
+        return np.stack([t.cpu().numpy() for t in g], 1)
+    finally:
+        ctx.close()
+
+
+def _rel(got, ref):
+    return np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)
+
+
+def _check(got, ref, idx, w, precision, label):
+    e = _rel(got[idx], ref)
+    assert np.all(np.isfinite(e)), label
+    rms = float(np.sqrt(np.mean(e ** 2)))
+    print("\n[fullsize] %s: N=%d targets=%d max rel err %.3e rms %.3e" % (label, w.n, len(idx), e.max(), rms))
+    if precision == 0:
+        assert e.max() <= FP64_TOL, "%s: fp64 max rel err %.3e" % (label, e.max())
+    else:
+        assert rms <= MIXED_RMS and e.max() <= MIXED_MAX, "%s: mixed rms %.3e max %.3e" % (label, rms, e.max())
+    # momentum conservation over ALL particles (pair antisymmetry): holds at any size
+    for c in range(3):
+        assert abs(np.sum(w.m * got[:, c])) <= (1e-11 if precision == 0 else 1e-5) * np.sum(w.m * np.abs(got[:, c])), label
+
+
+@pytest.fixture(scope="module")
+def cfg_case():
+    """(workload, target indices, oracle accelerations) per config, built once per module."""
+    cache = {}
+
+    def get(cfg, k, oracle):
+        if cfg not in cache:
+            from paper_2602_20787_b200 import workloads
+            w = workloads.make(cfg, n=workloads.CONFIG_N[cfg] // SCALE)
+            idx = _targets(w, cfg, k)
+            ref = np.stack(oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, w.n_cut, targets=idx), 1)
+            cache[cfg] = (w, idx, ref)
+        return cache[cfg]
+    return get
+
+
+MODES = [("fp64", 0, 0), ("mixed", 1, 0), ("fp64_deterministic", 0, 1)]
+
+
+@pytest.mark.parametrize("name,precision,flags", MODES, ids=[m[0] for m in MODES])
+def test_config2_full_size(torch_cuda, oracle, cfg_case, name, precision, flags):
+    """BASELINE configs[2]: N = 262 144 compactified layout + Zel'dovich displacements, fp64 and mixed."""
+    w, idx, ref = cfg_case(2, 1024, oracle)
+    assert SCALE > 1 or w.n == 262144
+    _check(_accel(torch_cuda, w, precision, flags), ref, idx, w, precision, "cfg2 " + name)
+
+
+@pytest.mark.parametrize("name,precision,flags", MODES, ids=[m[0] for m in MODES])
+def test_config4_full_size(torch_cuda, oracle, cfg_case, name, precision, flags):
+    """BASELINE configs[4]: N = 4 194 304, 512 Plummer spheres + 20 % compactified background; half of the
+    sampled targets sit inside spheres (softened pairs in both spline branches, spheres straddling z = 0 / L)."""
+    w, idx, ref = cfg_case(4, 256, oracle)
+    assert SCALE > 1 or w.n == 4194304
+    ncl = w.cosmo["n_clustered"]
+    assert (idx < ncl).sum() == 128 and (idx >= ncl).sum() == 128
+    _check(_accel(torch_cuda, w, precision, flags), ref, idx, w, precision, "cfg4 " + name)
+
+
+def test_config3_full_size_step0_and_step10(torch_cuda, oracle, cfg_case):
+    """BASELINE configs[3]: N = 1 048 576, LCDM background, 10 KDK steps a = 0.02 -> 0.025 on the GPU.
+    g is compared with the oracle at step 0 and -- on the GPU's own step-10 positions, copied back -- at
+    step 10.  The trajectory itself (oracle integrating independently) is
+    test_gpu_kdk.py::test_config3_trajectory_reduced_n."""
+    from paper_2602_20787_b200 import binding as b
+    torch = torch_cuda
+    w, idx, ref0 = cfg_case(3, 192, oracle)
+    assert SCALE > 1 or w.n == 1048576
+    c = w.cosmo
+    names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
+    dev = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k), dtype=np.float64)).cuda() for k in names}
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=w.n_cut, R_sim=w.R_sim, rho0=w.rho0)
+    try:
+        ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+        ctx.check()
+        _check(np.stack([t.cpu().numpy() for t in g], 1), ref0, idx, w, 0, "cfg3 step 0")
+        a = c["a_init"]
+        _, H = b.friedmann_step(a, 0.0, c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+        for _ in range(c["n_steps"]):
+            a1, H1 = b.friedmann_step(a, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+            ctx.kdk_step(*[dev[k] for k in names], *g, a, H, a1, H1, c["dt"])
+            a, H = a1, H1
+        ctx.check()
+    finally:
+        ctx.close()
+    assert a == pytest.approx(c["a_final"], rel=1e-6)
+    x10, y10, z10 = (dev[k].cpu().numpy() for k in ("x", "y", "z"))
+    # the particles moved (a fraction of the inner grid spacing) and stayed inside [0, L)
+    moved = np.sqrt((x10 - w.x) ** 2 + (y10 - w.y) ** 2)
+    assert np.median(moved[np.hypot(w.x, w.y) < 20.0]) > 1e-3 * c["d0"]
+    assert z10.min() >= 0.0 and z10.max() < w.Lz
+    ref10 = np.stack(oracle.accel(x10, y10, z10, w.m, w.h, w.Lz, w.G, w.n_cut, targets=idx), 1)
+    assert _rel(ref10, ref0).max() > 1e-6          # a different state, not step 0 again
+    got10 = np.stack([t.cpu().numpy() for t in g], 1)
+    _check(got10, ref10, idx, w, 0, "cfg3 step 10")
+
+
+def test_config3_full_size_deterministic(torch_cuda, oracle, cfg_case):
+    """STEPS_FLAG_DETERMINISTIC at the bench size (4098 round launches per evaluation at N = 1 048 576)."""
+    w, idx, ref0 = cfg_case(3, 192, oracle)
+    _check(_accel(torch_cuda, w, 0, 1), ref0, idx, w, 0, "cfg3 fp64_deterministic")
