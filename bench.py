@@ -238,6 +238,10 @@ def roofline_of(ctx, n, n_cut, t_pair, sm_count, sm_max, table):
     if is_mixed or cnt["fp32_ops"] > 0:
         xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
         r["xu_pipe_util_vs_nominal"] = (cnt["mufu"] + cnt["conv"]) * pairs / t_pair / xu_peak
+    if not np.isfinite(t_pair):      # STEPS_FLAG_GRAPH: the kernel is not timed on its own inside the graph
+        for key in ("achieved", "frac", "pipe_util_vs_nominal", "kernel_ms", "xu_pipe_util_vs_nominal"):
+            if key in r:
+                r[key] = None
     return r
 
 
@@ -300,20 +304,32 @@ def run_ours(args):
         sampler = ClockSampler(local)
         if rank == 0 and sample_clocks:
             sampler.start()
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        # device time of each step: a CUDA event pair around the step on the launching stream, the L2 flush between
+        # steps outside it.  Large N: the pair kernel's own events are read after every step (a host sync that costs
+        # nothing against seconds of kernel); small N: no host sync inside the loop, the last step's pair time is read.
+        graph = bool(flags & b.FLAG_GRAPH)
+        sync_each = n >= 100000 and not graph
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         pair_ms = []
-        ev[0].record()
         for k in range(steps):
-            step(warmup + k)
-            pair_ms.append(ctx.last_pair_kernel_ms())          # waits for that launch's end event
-        ev[1].record()
+            flush.zero_()
+            evs[k][0].record()
+            ctx.kdk_step(*[dev[q] for q in names], *g, *sched[warmup + k], w.cosmo["dt"])
+            evs[k][1].record()
+            if sync_each:
+                pair_ms.append(ctx.last_pair_kernel_ms())          # waits for that launch's end event
         barrier()
+        if not sync_each and not graph:
+            pair_ms.append(ctx.last_pair_kernel_ms())
         clocks = sampler.stop() if (rank == 0 and sample_clocks) else {}
         ctx.check()
-        t_dev = max_over_ranks(ev[0].elapsed_time(ev[1]) * 1e-3, dist, "cuda")
+        step_ms = [e0.elapsed_time(e1) for e0, e1 in evs]
+        t_dev = max_over_ranks(float(np.sum(step_ms)) * 1e-3, dist, "cuda")
+        if not pair_ms:
+            pair_ms = [float("nan")]
         out = {"ctx": ctx, "t_dev": t_dev, "t_pair": float(np.mean(pair_ms)) * 1e-3, "clocks": clocks,
                "launches_per_step": launches_per_step, "value": replica_throughput(pairs_per_step, steps, world, t_dev),
-               "e2e_value": None}
+               "e2e_value": None, "step_ms_min": float(np.min(step_ms)), "step_ms_median": float(np.median(step_ms))}
         if e2e_steps:
             # end to end: pinned host buffers through steps_cyl_kdk_step_host, copies inside the timing
             hs = [host[q] for q in names] + hg
@@ -352,8 +368,8 @@ def run_ours(args):
         return
     t_dev, t_pair = main["t_dev"], main["t_pair"]
     roofline = roofline_of(ctx, n, args.n_cut, t_pair, sm_count, sm_max, table)
-    roofline["kernel_share_of_step"] = t_pair * args.steps / t_dev
-    if "mixed" not in roofline["kernel"]:
+    roofline["kernel_share_of_step"] = t_pair * args.steps / t_dev if np.isfinite(t_pair) else None
+    if "mixed" not in roofline["kernel"] and np.isfinite(t_pair):
         roofline["measured_dfma_tflops"] = 2 * dfma_per_s / 1e12
         roofline["pipe_util_vs_measured_dfma"] = (roofline["pipe_instr_per_pair_interaction"] * pairs_per_step
                                                   / t_pair / dfma_per_s)
@@ -398,9 +414,11 @@ def run_ours(args):
         "config": {"workload": "BASELINE configs[3]: N=%d LCDM comoving KDK step (Om=0.3, OL=0.7, "
                                "a 0.02->0.025), L=100 Mpc/h, r_max=1000, %s" % (n, periodic_desc),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "256 MiB buffer written between steps (L2 flush)"},
+                   "l2": "256 MiB buffer written between steps (L2 flush), outside the per-step event pairs",
+                   "graph": bool(args.graph)},
         "image_terms_per_s": None if table else main["value"] * 2 * args.n_cut,
-        "seconds_per_force_evaluation": t_pair,
+        "seconds_per_force_evaluation": t_pair if np.isfinite(t_pair) else None, "step_ms_min": main["step_ms_min"],
+        "step_ms_median": main["step_ms_median"],
         "roofline": roofline, "cpu_baseline": cpu, "clocks": main["clocks"],
         "e2e": {"value": main["e2e_value"], "unit": "pairs/s", "h2d_bytes_per_step": 11 * 8 * n,
                 "d2h_bytes_per_step": 9 * 8 * n},

@@ -81,9 +81,13 @@ enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,
                                           per-particle error <~ 2e-12 instead of ~1e-14 (bar: 1e-10)  */
-       STEPS_FLAG_ORDERED_PAIRS = 4    /* fp64 / mixed images mode: the literal form of Eq. 1 -- every target
+       STEPS_FLAG_ORDERED_PAIRS = 4,   /* fp64 / mixed images mode: the literal form of Eq. 1 -- every target
                                           sums over all its sources (ordered pairs, fixed-order reduction,
-                                          bit-reproducible, ~1.9x slower than the default)             */ };
+                                          bit-reproducible, ~1.9x slower than the default)             */
+       STEPS_FLAG_GRAPH = 8            /* steps_cyl_accel / steps_cyl_kdk_step replay a CUDA graph captured on the
+                                          first call with a given set of array pointers (one launch per call
+                                          instead of three: small-N step latency); same kernels, same results.
+                                          steps_cyl_last_pair_kernel_ms is not available in this mode  */ };
 
 /* Largest particle number one context takes: the symmetric kernels put chunks of <= 64 source tiles of 128
  * particles on gridDim.y (<= 65535).  (At 40 B/particle in and ~250 B/particle of scratch this is also

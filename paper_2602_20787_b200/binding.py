@@ -19,6 +19,7 @@ BG_FINITE, BG_INFINITE = 0, 1
 FLAG_DETERMINISTIC = 1
 FLAG_FAR_ORDER2 = 2
 FLAG_ORDERED_PAIRS = 4
+FLAG_GRAPH = 8
 INTERP_CIC, INTERP_TSC = 0, 1
 
 EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_accel_host",

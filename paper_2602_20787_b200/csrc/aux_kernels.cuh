@@ -18,80 +18,6 @@ __device__ __forceinline__ double wrap_z(double z, double L)
     return w;
 }
 
-// a1: SoA inputs -> packed, padded source arrays; records max(h) and h <= 0.
-// Mixed mode additionally gets float hi/lo splits (see pair_mixed.cuh).
-__global__ void pack_kernel(const double *__restrict__ x, const double *__restrict__ y,
-                            const double *__restrict__ z, const double *__restrict__ m,
-                            const double *__restrict__ h, int n, int n_pad, double L,
-                            double2 *__restrict__ xy, double2 *__restrict__ zm,
-                            double *__restrict__ hs,
-                            float4 *__restrict__ f_hi, float4 *__restrict__ f_lo,
-                            double *__restrict__ tile_hmax, DevFlags *__restrict__ flags)
-{
-    // launched with PAIR_THREADS threads per block: block b == source tile b (n_pad = tiles * 128)
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double xv, yv, zv, mv, hv;
-    if (i < n) {
-        xv = x[i]; yv = y[i]; zv = wrap_z(z[i], L); mv = m[i]; hv = h[i];
-        if (!(hv > 0.0)) atomicOr(&flags->bad_h, 1);
-        else atomicMax(&flags->hmax_bits, (unsigned long long)__double_as_longlong(hv));
-    } else {                   // massless dummy far outside any particle load
-        xv = 1.0e60; yv = 1.0e60; zv = 0.0; mv = 0.0; hv = 1.0;
-    }
-    xy[i] = make_double2(xv, yv);
-    zm[i] = make_double2(zv, mv);
-    hs[i] = hv;
-    {   // max h of the tile (dummies count as 0): bounds h_i + h_j in the pair kernels' spline pre-test
-        __shared__ double s_max[PAIR_THREADS / 32];
-        double hm = (i < n && hv > 0.0) ? hv : 0.0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) hm = fmax(hm, __shfl_xor_sync(0xffffffffu, hm, o));
-        if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = hm;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t = s_max[0];
-            for (int wq = 1; wq < PAIR_THREADS / 32; ++wq) t = fmax(t, s_max[wq]);
-            tile_hmax[blockIdx.x] = t;
-        }
-    }
-    if (f_hi) {
-        // x = hi + lo with hi = fl32(x), lo = fl32(x - hi): the difference of two such pairs,
-        // (hi_i - hi_j) + (lo_i - lo_j), keeps ~2^-24 RELATIVE accuracy of the separation
-        // even for close pairs at large radius (Sterbenz: the hi difference is then exact).
-        if (i >= n) { xv = 1.0e18; yv = 1.0e18; }
-        const float xh = (float)xv, yh = (float)yv, zh = (float)zv;
-        f_hi[i] = make_float4(xh, yh, zh, (float)mv);
-        f_lo[i] = make_float4((float)(xv - (double)xh), (float)(yv - (double)yh),
-                              (float)(zv - (double)zh), (float)hv);
-    }
-}
-
-// a5: g = -G (A_x, A_y, A_z1 - L A_z2), partial sums added over source chunks in fixed order.
-// n_chunks_fast: chunks written by the fast-path kernel that ran (1 for the symmetric kernel);
-// n_chunks_general: chunks of the general kernel, which ran instead iff 2 max(h) > L/2.
-__global__ void finalize_kernel(const double *__restrict__ part, int n, int n_pad,
-                                int n_chunks_fast, int n_chunks_general, double halfL,
-                                const DevFlags *__restrict__ flags, double G, double L,
-                                double *__restrict__ gx, double *__restrict__ gy,
-                                double *__restrict__ gz)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-    const int n_chunks = ((2.0 * hmax > halfL) || flags->bad_h) ? n_chunks_general : n_chunks_fast;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    for (int c = 0; c < n_chunks; ++c) {
-        const double *p = part + (size_t)c * 4 * n_pad + i;
-        a0 += p[0];
-        a1 += p[(size_t)n_pad];
-        a2 += p[2 * (size_t)n_pad];
-        a3 += p[3 * (size_t)n_pad];
-    }
-    gx[i] = -G * a0;
-    gy[i] = -G * a1;
-    gz[i] = -G * fma(-L, a3, a2);
-}
-
 // a6: homogeneous cylinder, Eq. 9 in the corrected form of DESIGN.md reading G3:
 //   F_h = 2 G rho0 int_0^R { 2 ln[(w+ + L)/(w- + L)] - ln(a+/a-) } dY,
 //   a+- = R^2 + rho^2 +- 2 rho sqrt(R^2 - Y^2),  w+- = sqrt(L^2 + a+-),  L = N_cut L_z,
@@ -121,77 +47,187 @@ __device__ __forceinline__ double background_nodes(double rho, double R, double 
     return acc;
 }
 
-// LANES = 1: one thread per particle.  LANES = 32: one warp per particle (nodes strided over the lanes,
-// fixed-order butterfly sum) -- for small n, where one thread per particle leaves most SMs empty and the
-// 361-node loop (~120 us) would outlast the pair kernel.
+// ---------------------------------------------------------------------------------------------
+// The O(N) work of a force evaluation / KDK step is two launches around the all-pairs kernel:
+//   prestep_kernel  : [b(x_n), kick 1, drift]  pack + wrap (a1), zero the accumulators, max(h), h <= 0
+//   poststep_kernel : partial-sum reduction (a5)  [b(x_n+1), kick 2]
+// (the bracketed parts only inside steps_cyl_kdk_step).  One CTA per 128-particle tile.  LANES = 32: the CTA
+// has 32 warps and the Eq. 9 quadrature of each particle is spread over the lanes of a warp (small n, where one
+// thread per particle would leave most SMs empty for the 361-node loop); LANES = 1: 128 threads, one per particle.
+struct BgParams {
+    double R, Lhalf, G, rho0;
+    int infinite;                    // Eq. 10 instead of Eq. 9
+    int n_nodes;
+    const QuadNode *nodes;
+};
+struct KickParams { double inv_a3, H, dt; };
+
+// s with b = s (x, y): s = -F_h(rho)/rho (Eq. 11 subtracts F_h < 0: outward push); 0 when disabled or on the axis.
+// LANES == 32: called by a whole warp for ONE particle, every lane returns the sum.
+template <int LANES>
+__device__ __forceinline__ double background_scale(double xv, double yv, const BgParams &bg, int lane)
+{
+    if (bg.rho0 == 0.0) return 0.0;
+    const double rho = sqrt(fma(xv, xv, yv * yv));
+    if (rho == 0.0) return 0.0;
+    double Fh;
+    if (bg.infinite) {
+        Fh = -2.0 * 3.141592653589793238 * bg.G * bg.rho0 * rho;          // Eq. 10
+    } else {
+        double acc = background_nodes(rho, bg.R, bg.Lhalf, bg.nodes, bg.n_nodes, LANES == 32 ? lane : 0, LANES);
+        if (LANES == 32) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        }
+        Fh = 2.0 * bg.G * bg.rho0 * acc;
+    }
+    return -Fh / rho;
+}
+
+// Background scale of the tile's 128 particles into s_bg[128] (LANES == 32) or the caller's register.
+template <int LANES>
+__device__ __forceinline__ double tile_background(const double *__restrict__ x, const double *__restrict__ y,
+                                                  int tile, int n, const BgParams &bg, double *s_bg)
+{
+    if (LANES == 1) {
+        const int i = tile * PAIR_THREADS + threadIdx.x;
+        return (i < n) ? background_scale<1>(x[i], y[i], bg, 0) : 0.0;
+    }
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll 1
+    for (int q = 0; q < PAIR_THREADS / 32; ++q) {                      // 32 warps x 4 particles
+        const int p = w * (PAIR_THREADS / 32) + q, i = tile * PAIR_THREADS + p;
+        const double sv = (i < n) ? background_scale<32>(x[i], y[i], bg, lane) : 0.0;      // i is warp-uniform
+        if (lane == 0) s_bg[p] = sv;
+    }
+    __syncthreads();
+    return (threadIdx.x < PAIR_THREADS) ? s_bg[threadIdx.x] : 0.0;
+}
+
+// a1 (+ a6, a7 first half when KICK).  KICK (reading S4):
+//   v <- v + (dt/2)[(g + b)/a_n^3 - 2 H_n v];  x <- x + v dt;  z reduced to [0, L)
+// then, for the positions the force is wanted at: SoA -> packed, padded source arrays (massless far-away dummies
+// beyond n), float hi/lo splits for the mixed kernels, per-tile max h (bounds h_i + h_j in the spline pre-test),
+// global max h and the h <= 0 flag, and zeroed accumulator rows part[0 .. zero_rows) x [n_pad].
+template <int LANES, bool KICK>
+__global__ void __launch_bounds__(LANES == 32 ? 1024 : PAIR_THREADS)
+prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restrict__ z,
+               double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
+               const double *__restrict__ gx, const double *__restrict__ gy, const double *__restrict__ gz,
+               const double *__restrict__ m, const double *__restrict__ h, int n, int n_pad, double L,
+               BgParams bg, KickParams kp,
+               double2 *__restrict__ xy, double2 *__restrict__ zm, double *__restrict__ hs,
+               float4 *__restrict__ f_hi, float4 *__restrict__ f_lo, double *__restrict__ tile_hmax,
+               DevFlags *__restrict__ flags, int *__restrict__ bad_h_sticky,
+               double *__restrict__ part, int zero_rows)
+{
+    __shared__ double s_bg[PAIR_THREADS];
+    __shared__ double s_max[PAIR_THREADS / 32];
+    double sb = 0.0;
+    if (KICK) sb = tile_background<LANES>(x, y, blockIdx.x, n, bg, s_bg);
+    if (threadIdx.x >= PAIR_THREADS) return;
+    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
+    double xv, yv, zv, mv, hv;
+    if (i < n) {
+        xv = x[i]; yv = y[i]; zv = z[i]; mv = m[i]; hv = h[i];
+        if (KICK) {
+            const double hdt = 0.5 * kp.dt;
+            double ux = vx[i], uy = vy[i], uz = vz[i];
+            ux = ux + hdt * ((gx[i] + sb * xv) * kp.inv_a3 - 2.0 * kp.H * ux);
+            uy = uy + hdt * ((gy[i] + sb * yv) * kp.inv_a3 - 2.0 * kp.H * uy);
+            uz = uz + hdt * (gz[i] * kp.inv_a3 - 2.0 * kp.H * uz);
+            vx[i] = ux; vy[i] = uy; vz[i] = uz;
+            xv = xv + ux * kp.dt;
+            yv = yv + uy * kp.dt;
+            zv = wrap_z(zv + uz * kp.dt, L);
+            x[i] = xv; y[i] = yv; z[i] = zv;
+        } else {
+            zv = wrap_z(zv, L);
+        }
+        if (!(hv > 0.0)) { atomicOr(&flags->bad_h, 1); atomicOr(bad_h_sticky, 1); }
+        else atomicMax(&flags->hmax_bits, (unsigned long long)__double_as_longlong(hv));
+    } else {                   // massless dummy far outside any particle load
+        xv = 1.0e60; yv = 1.0e60; zv = 0.0; mv = 0.0; hv = 1.0;
+    }
+    xy[i] = make_double2(xv, yv);
+    zm[i] = make_double2(zv, mv);
+    hs[i] = hv;
+    for (int r = 0; r < zero_rows; ++r) part[(size_t)r * n_pad + i] = 0.0;
+    {   // max h of the tile (dummies count as 0)
+        double hm = (i < n && hv > 0.0) ? hv : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) hm = fmax(hm, __shfl_xor_sync(0xffffffffu, hm, o));
+        if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = hm;
+        // only the first four warps are here: a named barrier over them (bar 1), not __syncthreads
+        asm volatile("bar.sync 1, %0;" ::"n"(PAIR_THREADS));
+        if (threadIdx.x == 0) {
+            double t = s_max[0];
+            for (int wq = 1; wq < PAIR_THREADS / 32; ++wq) t = fmax(t, s_max[wq]);
+            tile_hmax[blockIdx.x] = t;
+        }
+    }
+    if (f_hi) {
+        // x = hi + lo with hi = fl32(x), lo = fl32(x - hi): the difference of two such pairs,
+        // (hi_i - hi_j) + (lo_i - lo_j), keeps ~2^-24 RELATIVE accuracy of the separation
+        // even for close pairs at large radius (Sterbenz: the hi difference is then exact).
+        if (i >= n) { xv = 1.0e18; yv = 1.0e18; }
+        const float xh = (float)xv, yh = (float)yv, zh = (float)zv;
+        f_hi[i] = make_float4(xh, yh, zh, (float)mv);
+        f_lo[i] = make_float4((float)(xv - (double)xh), (float)(yv - (double)yh),
+                              (float)(zv - (double)zh), (float)hv);
+    }
+}
+
+// a5 (+ a6, a7 second half when KICK): g = -G (A_x, A_y, A_z1 - L A_z2), the partial sums added over the n_slabs
+// slabs the pair kernel wrote, in fixed order; KICK:  v <- [v + (dt/2)(g' + b')/a_{n+1}^3] / (1 + H_{n+1} dt).
+// Also clears the flag block the NEXT call's prestep will use (flags alternate between two blocks, so that no
+// memset sits between the launches).
+template <int LANES, bool KICK>
+__global__ void __launch_bounds__(LANES == 32 ? 1024 : PAIR_THREADS)
+poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, double G, double L,
+                DevFlags *__restrict__ flags_next,
+                double *__restrict__ gx, double *__restrict__ gy, double *__restrict__ gz,
+                const double *__restrict__ x, const double *__restrict__ y,
+                double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
+                BgParams bg, KickParams kp)
+{
+    __shared__ double s_bg[PAIR_THREADS];
+    if (blockIdx.x == 0 && threadIdx.x == 0) { flags_next->hmax_bits = 0ull; flags_next->bad_h = 0; }
+    double sb = 0.0;
+    if (KICK) sb = tile_background<LANES>(x, y, blockIdx.x, n, bg, s_bg);
+    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
+    if (threadIdx.x >= PAIR_THREADS || i >= n) return;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    for (int c = 0; c < n_slabs; ++c) {
+        const double *p = part + (size_t)c * 4 * n_pad + i;
+        a0 += p[0];
+        a1 += p[(size_t)n_pad];
+        a2 += p[2 * (size_t)n_pad];
+        a3 += p[3 * (size_t)n_pad];
+    }
+    const double g0 = -G * a0, g1 = -G * a1, g2 = -G * fma(-L, a3, a2);
+    gx[i] = g0; gy[i] = g1; gz[i] = g2;
+    if (KICK) {
+        const double hdt = 0.5 * kp.dt, den = 1.0 + kp.H * kp.dt;
+        vx[i] = (vx[i] + hdt * (g0 + sb * x[i]) * kp.inv_a3) / den;
+        vy[i] = (vy[i] + hdt * (g1 + sb * y[i]) * kp.inv_a3) / den;
+        vz[i] = (vz[i] + hdt * g2 * kp.inv_a3) / den;
+    }
+}
+
+// steps_cyl_background: LANES = 1: one thread per particle.  LANES = 32: one warp per particle.
 template <int LANES>
 __global__ void background_kernel(const double *__restrict__ x, const double *__restrict__ y,
-                                  int n, double R, double Lhalf, double G, double rho0,
-                                  int infinite, const QuadNode *__restrict__ nodes, int n_nodes,
-                                  double *__restrict__ bx, double *__restrict__ by)
+                                  int n, BgParams bg, double *__restrict__ bx, double *__restrict__ by)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = tid / LANES, lane = tid % LANES;
     if (i >= n) return;                                               // uniform over a warp when LANES == 32
     const double xv = x[i], yv = y[i];
-    const double rho = sqrt(fma(xv, xv, yv * yv));
-    if (rho0 == 0.0 || rho == 0.0) {
-        if (lane == 0) { bx[i] = 0.0; by[i] = 0.0; }
-        return;
-    }
-    double Fh;
-    if (infinite) {
-        Fh = -2.0 * 3.141592653589793238 * G * rho0 * rho;          // Eq. 10
-    } else {
-        double acc = background_nodes(rho, R, Lhalf, nodes, n_nodes, lane, LANES);
-        if (LANES == 32) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        }
-        Fh = 2.0 * G * rho0 * acc;
-    }
+    const double s = background_scale<LANES>(xv, yv, bg, lane);
     if (lane != 0) return;
-    const double s = -Fh / rho;      // Eq. 11 subtracts F_h (F_h < 0): outward push
     bx[i] = s * xv;
     by[i] = s * yv;
-}
-
-// a7, first half of the KDK step (reading S4):
-//   v <- v + (dt/2)[(g + b)/a_n^3 - 2 H_n v];  x <- x + v dt;  z reduced to [0, L).
-__global__ void kick1_drift_kernel(double *__restrict__ x, double *__restrict__ y,
-                                   double *__restrict__ z, double *__restrict__ vx,
-                                   double *__restrict__ vy, double *__restrict__ vz,
-                                   const double *__restrict__ gx, const double *__restrict__ gy,
-                                   const double *__restrict__ gz, const double *__restrict__ bx,
-                                   const double *__restrict__ by, int n, double inv_a3,
-                                   double H, double dt, double L)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double hdt = 0.5 * dt;
-    double ux = vx[i], uy = vy[i], uz = vz[i];
-    ux = ux + hdt * ((gx[i] + bx[i]) * inv_a3 - 2.0 * H * ux);
-    uy = uy + hdt * ((gy[i] + by[i]) * inv_a3 - 2.0 * H * uy);
-    uz = uz + hdt * (gz[i] * inv_a3 - 2.0 * H * uz);
-    vx[i] = ux; vy[i] = uy; vz[i] = uz;
-    x[i] = x[i] + ux * dt;
-    y[i] = y[i] + uy * dt;
-    z[i] = wrap_z(z[i] + uz * dt, L);
-}
-
-// a7, second half:  v <- [v + (dt/2)(g' + b')/a_{n+1}^3] / (1 + H_{n+1} dt).
-__global__ void kick2_kernel(double *__restrict__ vx, double *__restrict__ vy,
-                             double *__restrict__ vz, const double *__restrict__ gx,
-                             const double *__restrict__ gy, const double *__restrict__ gz,
-                             const double *__restrict__ bx, const double *__restrict__ by, int n,
-                             double inv_a3, double H, double dt)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double hdt = 0.5 * dt, den = 1.0 + H * dt;
-    vx[i] = (vx[i] + hdt * (gx[i] + bx[i]) * inv_a3) / den;
-    vy[i] = (vy[i] + hdt * (gy[i] + by[i]) * inv_a3) / den;
-    vz[i] = (vz[i] + hdt * gz[i] * inv_a3) / den;
 }
 
 // FP64-pipe ceiling: 16 independent DFMA chains per thread, `iters` x 16 DFMAs each.

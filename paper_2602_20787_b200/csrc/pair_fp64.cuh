@@ -36,10 +36,12 @@ constexpr int kRtUnroll = STEPS_RT_UNROLL;      // image-loop unroll of the run-
                                                 // N_cut = 10: 490 / 478 / 480 / 486 ms per evaluation at N = 262144)
 constexpr int MAX_NCUT_TABLE = 64;  // run-time N_cut up to here reads its per-image constants from PairConsts
 
-struct PairConsts {
+struct WrapConsts {           // what the nearest-image reduction needs (all the general path reads)
     double L;                 // period
     double halfL;
     int L_hi, L_lo, halfL_hi; // integer views of L and L/2 (ALU-pipe wrap test)
+};
+struct PairConsts : WrapConsts {
     double c2nL[MAX_NCUT_TABLE + 1];      // 2 n L
     double n2L2[MAX_NCUT_TABLE + 1];      // (n L)^2
     double dn[MAX_NCUT_TABLE + 1];        // n
@@ -114,7 +116,7 @@ __device__ __forceinline__ int lo32(double v) { return __double2loint(v); }
 // Pair geometry (a2): r = x_i - x_j with r_z brought to the nearest image.  The decision uses
 // the high word only: |r_z| may stay above L/2 by a relative 2^-20, which leaves the image SET
 // {d = r_z - nL : |d| < N_cut L} and every formula below unchanged (reading S2).
-__device__ __forceinline__ double nearest_image(double rz, const PairConsts &k)
+__device__ __forceinline__ double nearest_image(double rz, const WrapConsts &k)
 {
     const int h = hi32(rz);
     const bool wrap = (h & 0x7fffffff) > k.halfL_hi;
@@ -258,28 +260,36 @@ __device__ __forceinline__ void pair_term(double xi, double yi, double zi, doubl
     az2 = fma(mj, T, az2);
 }
 
-// General path (2 max(h) > L/2): every image is formed directly and sent through the
-// spline test, exactly as Eq. 8 is written.
+// General path (2 max(h) > L/2, reading S7): every image of the window of Eq. 8 is formed directly and sent
+// through the spline test, exactly as the equation is written.  S = sum_n w_n, T = sum_n n w_n as in image_sum.
+__device__ __forceinline__ void image_sum_general(double rz, double rho2, double hh, const WrapConsts &k,
+                                                  int ncut, double &S, double &T)
+{
+    const double hh2 = hh * hh;
+    int nlo = -ncut + 1, nhi = ncut - 1;
+    if (rz > 0.0) nhi = ncut;
+    if (rz < 0.0) nlo = -ncut;
+    S = 0.0;
+    T = 0.0;
+    for (int n = nlo; n <= nhi; ++n) {
+        const double d = rz - (double)n * k.L;
+        const double s2 = fma(d, d, rho2);
+        const double w = (s2 < hh2) ? spline_w(s2, hh) : inv_cube_sqrt(s2);
+        S += w;
+        T = fma((double)n, w, T);
+    }
+}
+
 __device__ __forceinline__ void pair_term_general(double xi, double yi, double zi, double hi,
                                                   double xj, double yj, double zj, double mj,
-                                                  double hj, const PairConsts &k, int ncut,
+                                                  double hj, const WrapConsts &k, int ncut,
                                                   double &ax, double &ay, double &az1, double &az2)
 {
     const double rx = xi - xj, ry = yi - yj;
     const double rz = nearest_image(zi - zj, k);
     const double rho2 = fma(ry, ry, rx * rx);
-    const double hh = hi + hj, hh2 = hh * hh;
-    int nlo = -ncut + 1, nhi = ncut - 1;
-    if (rz > 0.0) nhi = ncut;
-    if (rz < 0.0) nlo = -ncut;
-    double S = 0.0, T = 0.0;
-    for (int n = nlo; n <= nhi; ++n) {
-        const double d = rz - (double)n * k.L;
-        const double s2 = fma(d, d, rho2);
-        double w = (s2 < hh2) ? spline_w(s2, hh) : inv_cube_sqrt(s2);
-        S += w;
-        T = fma((double)n, w, T);
-    }
+    double S, T;
+    image_sum_general(rz, rho2, hi + hj, k, ncut, S, T);
     const double Sm = mj * S;
     ax  = fma(Sm, rx, ax);
     ay  = fma(Sm, ry, ay);
@@ -287,30 +297,28 @@ __device__ __forceinline__ void pair_term_general(double xi, double yi, double z
     az2 = fma(mj, T, az2);
 }
 
-// Packed source layout (written by pack_kernel, padded to a multiple of PAIR_THREADS with
+// True when the fast kernels' precondition fails: some far image can fall inside a spline support
+// (2 max h > L/2), or some h <= 0 (outputs then unspecified, reported through steps_cyl_check).
+__device__ __forceinline__ bool need_general_path(const DevFlags *flags, double halfL)
+{
+    const double hmax = __longlong_as_double((long long)flags->hmax_bits);
+    return (2.0 * hmax > halfL) || flags->bad_h;
+}
+
+// Packed source layout (written by prestep_kernel, padded to a multiple of PAIR_THREADS with
 // massless far-away dummies): xy[j] = {x, y}, zm[j] = {z in [0,L), m}, hs[j] = h.
 //
-// grid = (ceil(n / PAIR_THREADS), n_chunks); CTA (bx, by) handles targets
-// [bx*128, bx*128+128) against source tiles [by*tiles_per_chunk, (by+1)*tiles_per_chunk).
+// Ordered pairs, the literal form of Eq. 1 (STEPS_FLAG_ORDERED_PAIRS): grid = (n_tiles, n_chunks); CTA (bx, by)
+// handles targets [bx*128, bx*128+128) against source tiles [by*tiles_per_chunk, (by+1)*tiles_per_chunk).
 // part layout: part[((chunk*4 + comp) * n_pad) + i].
-// MODE: 0 = fast path (exits at once if the general path is required), 1 = general path
-// (exits at once if it is not).
-template <int NC, int MODE>
-__global__ void __launch_bounds__(PAIR_THREADS)
-pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
-                 const double *__restrict__ hs, const double *__restrict__ tile_hmax, int n_pad,
-                 int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
-                 const DevFlags *__restrict__ flags, double *__restrict__ part)
-{
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        const bool need_general = (2.0 * hmax > k.halfL) || flags->bad_h;
-        if (need_general != (MODE == 1)) return;
-    }
-    __shared__ double2 s_xy[PAIR_THREADS];
-    __shared__ double2 s_zm[PAIR_THREADS];
-    __shared__ double  s_h[PAIR_THREADS];
+struct OrdSmem { double2 xy[PAIR_THREADS]; double2 zm[PAIR_THREADS]; double h[PAIR_THREADS]; };
 
+template <int NC, bool GENERAL, class KC>
+__device__ __forceinline__ void ordered_body(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                                             const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                                             int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt,
+                                             const KC &k, double *__restrict__ part, OrdSmem &sm)
+{
     const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;      // < n_pad always
     const double2 pi = xy[i], qi = zm[i];
     const double xi = pi.x, yi = pi.y, zi = qi.x, hi = hs[i];
@@ -321,9 +329,9 @@ pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
     for (int t = t0; t < t1; ++t) {
         const int j = t * PAIR_THREADS + threadIdx.x;
         __syncthreads();
-        s_xy[threadIdx.x] = xy[j];
-        s_zm[threadIdx.x] = zm[j];
-        s_h[threadIdx.x]  = hs[j];
+        sm.xy[threadIdx.x] = xy[j];
+        sm.zm[threadIdx.x] = zm[j];
+        sm.h[threadIdx.x]  = hs[j];
         __syncthreads();
         int soft_hi;
         {
@@ -332,14 +340,12 @@ pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
         }
 #pragma unroll 1
         for (int jj = 0; jj < PAIR_THREADS; ++jj) {
-            const double2 a = s_xy[jj], b = s_zm[jj];
-            const double hj = s_h[jj];
-            if (MODE == 0)
-                pair_term<NC>(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, soft_hi, k, ncut_rt, ax, ay, az1,
-                              az2);
+            const double2 a = sm.xy[jj], b = sm.zm[jj];
+            const double hj = sm.h[jj];
+            if constexpr (GENERAL)
+                pair_term_general(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt, ax, ay, az1, az2);
             else
-                pair_term_general(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, k, ncut_rt,
-                                  ax, ay, az1, az2);
+                pair_term<NC>(xi, yi, zi, hi, a.x, a.y, b.x, b.y, hj, soft_hi, k, ncut_rt, ax, ay, az1, az2);
         }
     }
     double *p = part + (size_t)blockIdx.y * 4 * n_pad + i;
@@ -347,6 +353,30 @@ pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
     p[(size_t)n_pad] = ay;
     p[2 * (size_t)n_pad] = az1;
     p[3 * (size_t)n_pad] = az2;
+}
+
+// The general path of the ordered kernels (fp64 and mixed), out of line so that it costs the fast path nothing.
+__device__ __noinline__ void ordered_body_general(const double2 *xy, const double2 *zm, const double *hs,
+                                                  const double *tile_hmax, int n_pad, int n_tiles,
+                                                  int tiles_per_chunk, int ncut_rt, WrapConsts k,
+                                                  double *part, OrdSmem &sm)
+{
+    ordered_body<0, true>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, part, sm);
+}
+
+template <int NC>
+__global__ void __launch_bounds__(PAIR_THREADS)
+pair_fp64_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                 const double *__restrict__ hs, const double *__restrict__ tile_hmax, int n_pad,
+                 int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
+                 const DevFlags *__restrict__ flags, double *__restrict__ part)
+{
+    __shared__ OrdSmem sm;
+    if (need_general_path(flags, k.halfL)) {
+        ordered_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, part, sm);
+        return;
+    }
+    ordered_body<NC, false>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, part, sm);
 }
 
 }  // namespace steps

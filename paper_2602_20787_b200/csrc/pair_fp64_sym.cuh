@@ -26,6 +26,10 @@
 // Results are accumulated with floating-point atomics, so the summation ORDER (not the set of
 // terms) can differ from run to run: results are reproducible to round-off (~1e-16 relative),
 // not bit for bit.  STEPS_FLAG_DETERMINISTIC selects pair_fp64_round_kernel (end of this file).
+//
+// If 2 max(h) > L/2 (a far image can be softened, reading S7) the same CTA runs the general pair law instead --
+// same ring, same decomposition, every image through the spline test -- decided on the device from the flag
+// block prestep_kernel wrote.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -52,9 +56,9 @@ struct SymTgt { double x, y, z, h, m, mL; };         // mL = -L m
 // pairs.  SYM: also accumulate on the sources.  Source-side accumulators (rotating):
 // bx = sum m_i S r_x, by = sum m_i S r_y, bz = sum m_i (S r_z - L T) -- z already combined,
 // so only three values travel.
-template <int NC, int R, bool SYM, bool O2>
+template <int NC, int R, bool SYM, bool O2, bool GENERAL = false, class KC = PairConsts>
 __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&soft_hi)[R],
-                                             const SymSrc *s_src, int lane, const PairConsts &k,
+                                             const SymSrc *s_src, int lane, const KC &k,
                                              int ncut_rt, double (&a)[R][4], double &bx,
                                              double &by, double &bz)
 {
@@ -65,7 +69,29 @@ __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&
         const double2 pa = *reinterpret_cast<const double2 *>(&sj->x);
         const double2 pb = *reinterpret_cast<const double2 *>(&sj->z);
         const double hj = sj->h;
-        if constexpr (NC == 0) {
+        if constexpr (GENERAL) {
+            // general path (2 max h > L/2): the literal image loop of Eq. 8 with every image through the spline
+            // test; (S, T) serve both particles of the pair exactly as on the fast path
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
+                const double rz = nearest_image(ti[r].z - pb.x, k);
+                double S, T;
+                image_sum_general(rz, fma(ry, ry, rx * rx), ti[r].h + hj, k, ncut_rt, S, T);
+                const double Sj = pb.y * S;
+                a[r][0] = fma(Sj, rx, a[r][0]);
+                a[r][1] = fma(Sj, ry, a[r][1]);
+                a[r][2] = fma(Sj, rz, a[r][2]);
+                a[r][3] = fma(pb.y, T, a[r][3]);
+                if (SYM) {
+                    const double Si = ti[r].m * S;
+                    bx = fma(Si, rx, bx);
+                    by = fma(Si, ry, by);
+                    bz = fma(Si, rz, bz);
+                    bz = fma(ti[r].mL, T, bz);
+                }
+            }
+        } else if constexpr (NC == 0) {
             // run-time N_cut: all R targets go through the image loop together (image_sum_rt)
             double rx[R], ry[R], rz[R], q[R], hi[R], S[R], T[R];
 #pragma unroll
@@ -128,27 +154,29 @@ __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&
 #endif
 constexpr int SYM_R = STEPS_SYM_R;     // target tiles per CTA (n_tiles is kept a multiple of SYM_R by the host)
 
-// acc layout: acc[comp * n_pad + particle], comp = 0..3 (A_x, A_y, A_z1, A_z2), zeroed by the host
+// Shared memory of a symmetric CTA: one staged source tile and the per-warp source accumulators.
+struct SymSmem {
+    SymSrc src[PAIR_THREADS];
+    double b[PAIR_THREADS / 32][3][PAIR_THREADS];
+};
+
+// acc layout: acc[comp * n_pad + particle], comp = 0..3 (A_x, A_y, A_z1, A_z2), zeroed by prestep_kernel
 // before the launch; the source side adds its combined z sum to A_z1.
 // grid = (n_tiles / SYM_R, chunks).  CTA (bi, c): target tiles SYM_R*bi + r (lane holds particle
 // tid of each), source tiles [c*tpc, (c+1)*tpc) from SYM_R*bi on.
-template <int NC, bool O2>
-__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
-pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
-                     const double *__restrict__ hs, const double *__restrict__ tile_hmax,
-                     int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
-                     const DevFlags *__restrict__ flags, double *__restrict__ acc)
+// GENERAL: the same decomposition with the general pair law (ring_subtile<..., GENERAL>).
+template <int NC, bool O2, bool GENERAL, class KC>
+__device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                                         const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                                         int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt,
+                                         const KC &k, double *__restrict__ acc, SymSmem &sm)
 {
     const int tb = blockIdx.x * SYM_R;                       // first target tile of this CTA
     const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        if ((2.0 * hmax > k.halfL) || flags->bad_h) return;      // general kernel's job
-    }
-    __shared__ SymSrc s_src[PAIR_THREADS];
-    __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];    // per-warp source accumulators
+    SymSrc *s_src = sm.src;
+    double (*s_b)[3][PAIR_THREADS] = sm.b;
 
     // gridDim.z == 4 (small N: fewer tile pairs than the GPU has schedulers): CTA z takes source sub-tile z only
     const bool split = gridDim.z == PAIR_THREADS / 32;
@@ -191,7 +219,7 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
             const SymSrc *sub = s_src + js * 32;
             if (t >= tb + SYM_R) {
                 // off-diagonal tile: every target of the CTA meets every source, both ways
-                ring_subtile<NC, SYM_R, true, O2>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+                ring_subtile<NC, SYM_R, true, O2, GENERAL, KC>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
             } else {
                 // one of the CTA's own tiles: target tile tb + r meets source tile t only if
                 // t >= tb + r; in its own tile (t == tb + r) warp w takes sub-tiles js > w both
@@ -204,9 +232,9 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
                     double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
                     double cx = 0.0, cy = 0.0, cz = 0.0;
                     if (tb + r < t || js > w)
-                        ring_subtile<NC, 1, true, O2>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                        ring_subtile<NC, 1, true, O2, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                     else if (js == w)
-                        ring_subtile<NC, 1, false, O2>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                        ring_subtile<NC, 1, false, O2, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                     bx += cx; by += cy; bz += cz;
                 }
             }
@@ -232,6 +260,30 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
     }
 }
 
+// The general path of the symmetric kernels (fp64 and mixed), out of line: it costs the fast path no registers.
+__device__ __noinline__ void sym_body_general(const double2 *xy, const double2 *zm, const double *hs,
+                                              const double *tile_hmax, int n_pad, int n_tiles,
+                                              int tiles_per_chunk, int ncut_rt, WrapConsts k,
+                                              double *acc, SymSmem &sm)
+{
+    sym_body<0, false, true>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+}
+
+template <int NC, bool O2>
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
+pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                     const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                     int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt, PairConsts k,
+                     const DevFlags *__restrict__ flags, double *__restrict__ acc)
+{
+    __shared__ SymSmem sm;
+    if (need_general_path(flags, k.halfL)) {          // decided on the device: no host synchronisation
+        sym_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+        return;
+    }
+    sym_body<NC, O2, false>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Deterministic variant (STEPS_FLAG_DETERMINISTIC): the same unordered-pair evaluation, scheduled in
 // ROUNDS so that no two CTAs ever update the same accumulator in one launch, and plain
@@ -245,13 +297,11 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
 // accumulator receives its contributions in a fixed order: bit-reproducible results at ~97 % of the
 // atomic kernel's speed (one tile of work per CTA per launch; T/2 + 2 launches per evaluation).
 // acc_i: gridDim.y slabs of [4][n_pad], acc_j: [3][n_pad], all zeroed by the host before round 0.
-template <int NC, bool SPLIT>
-__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
-pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
-                       const double *__restrict__ hs, const double *__restrict__ tile_hmax,
-                       int n_pad, int n_tiles, int round, int ncut_rt, PairConsts k,
-                       const DevFlags *__restrict__ flags, double *__restrict__ acc_i,
-                       double *__restrict__ acc_j)
+template <int NC, bool SPLIT, bool GENERAL, class KC>
+__device__ __forceinline__ void round_body(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                                           const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                                           int n_pad, int n_tiles, int round, int ncut_rt, const KC &k,
+                                           double *__restrict__ acc_i, double *__restrict__ acc_j, SymSmem &sm)
 {
     static_assert(SYM_R == 2, "round scheduling is written for two target tiles per CTA");
     const int tb = blockIdx.x * SYM_R;
@@ -266,12 +316,8 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
         }
     }
     if (mode[0] == 0 && mode[1] == 0) return;
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        if ((2.0 * hmax > k.halfL) || flags->bad_h) return;      // general kernel's job
-    }
-    __shared__ SymSrc s_src[PAIR_THREADS];
-    __shared__ double s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    SymSrc *s_src = sm.src;
+    double (*s_b)[3][PAIR_THREADS] = sm.b;
 
     // SPLIT (gridDim.y == 4; small N: a round has fewer items than the GPU has schedulers): CTA y takes source
     // sub-tile y only and adds its target-side sums into its own slab y of acc_i
@@ -305,7 +351,7 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
         double bx = 0.0, by = 0.0, bz = 0.0;
         const SymSrc *sub = s_src + js * 32;
         if (mode[0] == 1 && mode[1] == 1) {
-            ring_subtile<NC, SYM_R, true, false>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+            ring_subtile<NC, SYM_R, true, false, GENERAL, KC>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
         } else {
 #pragma unroll
             for (int r = 0; r < SYM_R; ++r) {
@@ -315,9 +361,9 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
                 double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
                 double cx = 0.0, cy = 0.0, cz = 0.0;
                 if (mode[r] == 1 || js > w)
-                    ring_subtile<NC, 1, true, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                    ring_subtile<NC, 1, true, false, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                 else if (js == w)
-                    ring_subtile<NC, 1, false, false>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
+                    ring_subtile<NC, 1, false, false, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
                 bx += cx; by += cy; bz += cz;
             }
         }
@@ -346,6 +392,32 @@ pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict
             *p = *p + a[r][c];
         }
     }
+}
+
+// The general path of the round-scheduled kernels (fp64 and mixed), out of line; bit-reproducible like the fast one.
+template <bool SPLIT>
+__device__ __noinline__ void round_body_general(const double2 *xy, const double2 *zm, const double *hs,
+                                                const double *tile_hmax, int n_pad, int n_tiles, int round,
+                                                int ncut_rt, WrapConsts k, double *acc_i, double *acc_j,
+                                                SymSmem &sm)
+{
+    round_body<0, SPLIT, true>(xy, zm, hs, tile_hmax, n_pad, n_tiles, round, ncut_rt, k, acc_i, acc_j, sm);
+}
+
+template <int NC, bool SPLIT>
+__global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
+pair_fp64_round_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                       const double *__restrict__ hs, const double *__restrict__ tile_hmax,
+                       int n_pad, int n_tiles, int round, int ncut_rt, PairConsts k,
+                       const DevFlags *__restrict__ flags, double *__restrict__ acc_i,
+                       double *__restrict__ acc_j)
+{
+    __shared__ SymSmem sm;
+    if (need_general_path(flags, k.halfL)) {
+        round_body_general<SPLIT>(xy, zm, hs, tile_hmax, n_pad, n_tiles, round, ncut_rt, k, acc_i, acc_j, sm);
+        return;
+    }
+    round_body<NC, SPLIT, false>(xy, zm, hs, tile_hmax, n_pad, n_tiles, round, ncut_rt, k, acc_i, acc_j, sm);
 }
 
 }  // namespace steps

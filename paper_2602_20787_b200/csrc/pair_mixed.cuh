@@ -136,20 +136,22 @@ __device__ __forceinline__ void pair_term_mixed(const float4 &ih, const float4 &
 }
 
 // Same grid / chunk / partial-sum layout as pair_fp64_kernel.  The fast path's precondition
-// (2 max h <= L/2) is required in mixed mode; otherwise the kernel exits and the fp64 general
-// kernel does the work.
+// (2 max h <= L/2) is required in mixed mode; otherwise the fp64 general path does the work (xy, zm, hs are
+// only read then).
 template <int NC>
 __global__ void __launch_bounds__(PAIR_THREADS)
-pair_mixed_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo, int n_pad,
-                  int n_tiles, int tiles_per_chunk, int ncut_rt, MixedConsts k, double halfL,
+pair_mixed_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
+                  const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                  const double *__restrict__ hs, const double *__restrict__ tile_hmax, int n_pad,
+                  int n_tiles, int tiles_per_chunk, int ncut_rt, MixedConsts k, PairConsts kd,
                   const DevFlags *__restrict__ flags, double *__restrict__ part)
 {
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        if ((2.0 * hmax > halfL) || flags->bad_h) return;
+    __shared__ OrdSmem sm;
+    if (need_general_path(flags, kd.halfL)) {
+        ordered_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, kd, part, sm);
+        return;
     }
-    __shared__ float4 s_hi[PAIR_THREADS];
-    __shared__ float4 s_lo[PAIR_THREADS];
+    float4 *s_hi = reinterpret_cast<float4 *>(sm.xy), *s_lo = reinterpret_cast<float4 *>(sm.zm);
     const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
     const float4 ih = f_hi[i], il = f_lo[i];
     double ax = 0.0, ay = 0.0, az1 = 0.0, az2 = 0.0;

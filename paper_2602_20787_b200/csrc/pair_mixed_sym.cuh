@@ -272,21 +272,23 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
 template <int NC>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
 pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
+                      const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                      const double *__restrict__ hs,
                       const double *__restrict__ tile_hmax, int n_pad, int n_tiles,
-                      int tiles_per_chunk, int ncut_rt, MixedConsts k, double halfL,
+                      int tiles_per_chunk, int ncut_rt, MixedConsts k, PairConsts kd,
                       const DevFlags *__restrict__ flags, double *__restrict__ acc)
 {
+    __shared__ SymSmem sm;
+    if (need_general_path(flags, kd.halfL)) {         // the fp64 general path (xy, zm, hs are only read here)
+        sym_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, kd, acc, sm);
+        return;
+    }
     const int tb = blockIdx.x * SYM_R;
     const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        if ((2.0 * hmax > halfL) || flags->bad_h) return;        // fp64 general kernel's job
-    }
-    __shared__ float4 s_hi[PAIR_THREADS];
-    __shared__ float4 s_lo[PAIR_THREADS];
-    __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    float4 *s_hi = reinterpret_cast<float4 *>(sm.src), *s_lo = s_hi + PAIR_THREADS;
+    float (*s_b)[3][PAIR_THREADS] = reinterpret_cast<float (*)[3][PAIR_THREADS]>(sm.b);
 
     // gridDim.z == 4 (small N): CTA z takes source sub-tile z only (see pair_fp64_sym_kernel)
     const bool split = gridDim.z == PAIR_THREADS / 32;
@@ -386,11 +388,18 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
 template <int NC, bool SPLIT>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
 pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict__ f_lo,
+                        const double2 *__restrict__ xy, const double2 *__restrict__ zm,
+                        const double *__restrict__ hs,
                         const double *__restrict__ tile_hmax, int n_pad, int n_tiles, int round,
-                        int ncut_rt, MixedConsts k, double halfL, const DevFlags *__restrict__ flags,
+                        int ncut_rt, MixedConsts k, PairConsts kd, const DevFlags *__restrict__ flags,
                         double *__restrict__ acc_i, double *__restrict__ acc_j)
 {
     static_assert(SYM_R == 2, "round scheduling is written for two target tiles per CTA");
+    __shared__ SymSmem sm;
+    if (need_general_path(flags, kd.halfL)) {         // the fp64 general path, same round scheduling
+        round_body_general<SPLIT>(xy, zm, hs, tile_hmax, n_pad, n_tiles, round, ncut_rt, kd, acc_i, acc_j, sm);
+        return;
+    }
     const int tb = blockIdx.x * SYM_R;
     const int t = (tb + round) % n_tiles;
     int mode[SYM_R];                                      // 0 skip, 1 both ways, 2 the tile against itself
@@ -403,13 +412,8 @@ pair_mixed_round_kernel(const float4 *__restrict__ f_hi, const float4 *__restric
         }
     }
     if (mode[0] == 0 && mode[1] == 0) return;
-    {
-        const double hmax = __longlong_as_double((long long)flags->hmax_bits);
-        if ((2.0 * hmax > halfL) || flags->bad_h) return;
-    }
-    __shared__ float4 s_hi[PAIR_THREADS];
-    __shared__ float4 s_lo[PAIR_THREADS];
-    __shared__ float  s_b[PAIR_THREADS / 32][3][PAIR_THREADS];
+    float4 *s_hi = reinterpret_cast<float4 *>(sm.src), *s_lo = s_hi + PAIR_THREADS;
+    float (*s_b)[3][PAIR_THREADS] = reinterpret_cast<float (*)[3][PAIR_THREADS]>(sm.b);
     // SPLIT (gridDim.y == 4): one source sub-tile per CTA, own acc_i slab (see pair_fp64_round_kernel)
     const int js0 = SPLIT ? blockIdx.y : 0, js1 = SPLIT ? blockIdx.y + 1 : PAIR_THREADS / 32;
     if (SPLIT) acc_i += (size_t)blockIdx.y * 4 * n_pad;

@@ -24,6 +24,14 @@
 
 using namespace steps;
 
+struct GraphSlot {
+    cudaGraphExec_t exec = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphNode_t pre = nullptr, post = nullptr;      // the prestep / poststep nodes (re-parameterised per step)
+    const void *key[11] = {};                           // the caller's pointers the graph was captured with
+    int n_kernels = 0;
+};
+
 struct steps_cyl_ctx {
     steps_cyl_params p;
     int n, n_pad, n_tiles;
@@ -41,8 +49,11 @@ struct steps_cyl_ctx {
     double *hs = nullptr, *tile_hmax = nullptr;
     float4 *f_hi = nullptr, *f_lo = nullptr;
     double *part = nullptr;
-    double *bx = nullptr, *by = nullptr;          // background acceleration at the current x
-    DevFlags *flags = nullptr;
+    DevFlags *flags = nullptr;                     // two blocks used by alternate force evaluations (+ a sticky word)
+    DevFlags *cur_flags = nullptr;                 // the block of the evaluation being enqueued
+    int *bad_h_sticky = nullptr;                   // h <= 0 seen since the last steps_cyl_check
+    unsigned eval_count = 0;
+    GraphSlot gslot[2];                            // STEPS_FLAG_GRAPH: one captured evaluation per flag-block parity
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
     float2 *d_table_f32 = nullptr;                 // the same rounded to float (tab_fp32), staged in smem
@@ -56,7 +67,6 @@ struct steps_cyl_ctx {
     cudaStream_t own_stream = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
-    bool bg_valid = false;                         // bx/by hold b(x) for the caller's current x
     int64_t launches = 0;
     char kernel_name[96];                          // the all-pairs kernel launch_pair() selects (sassmix.py naming)
     char cuda_msg[256];
@@ -176,9 +186,9 @@ template <int NC>
 void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles, c->n_chunks);
-    pair_fp64_kernel<NC, 0><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
+    pair_fp64_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
                                                          c->tiles_per_chunk, c->p.n_cut, c->kc,
-                                                         c->flags, c->part);
+                                                         c->cur_flags, c->part);
 }
 
 template <int NC>
@@ -189,12 +199,12 @@ void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
         pair_fp64_sym_kernel<NC, true><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
                                                                     c->n_pad, c->n_tiles,
                                                                     c->sym_tiles_per_chunk, c->p.n_cut,
-                                                                    c->kc, c->flags, c->part);
+                                                                    c->kc, c->cur_flags, c->part);
     else
         pair_fp64_sym_kernel<NC, false><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
                                                                      c->n_pad, c->n_tiles,
                                                                      c->sym_tiles_per_chunk, c->p.n_cut,
-                                                                     c->kc, c->flags, c->part);
+                                                                     c->kc, c->cur_flags, c->part);
 }
 
 // Deterministic fp64 path: rounds of the symmetric evaluation, one launch each (pair_fp64_sym.cuh).
@@ -206,12 +216,12 @@ void launch_pair_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
     for (int r = 0; r <= last; ++r) {
         if (c->round_split > 1)
             pair_fp64_round_kernel<NC, true><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(
-                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->flags, acc_i, acc_j);
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->cur_flags, acc_i, acc_j);
         else
             pair_fp64_round_kernel<NC, false><<<T / SYM_R, PAIR_THREADS, 0, s>>>(
-                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->flags, acc_i, acc_j);
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->kc, c->cur_flags, acc_i, acc_j);
     }
-    c->launches += last;      // launch_pair() adds the remaining 2
+    c->launches += last;      // launch_pair() adds the remaining one
 }
 
 template <int NC>
@@ -222,10 +232,12 @@ void launch_pair_mixed_rounds_nc(steps_cyl_ctx *c, cudaStream_t s)
     for (int r = 0; r <= last; ++r) {
         if (c->round_split > 1)
             pair_mixed_round_kernel<NC, true><<<dim3(T / SYM_R, c->round_split), PAIR_THREADS, 0, s>>>(
-                c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc.halfL, c->flags, acc_i, acc_j);
+                c->f_hi, c->f_lo, c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc, c->cur_flags,
+                acc_i, acc_j);
         else
             pair_mixed_round_kernel<NC, false><<<T / SYM_R, PAIR_THREADS, 0, s>>>(
-                c->f_hi, c->f_lo, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc.halfL, c->flags, acc_i, acc_j);
+                c->f_hi, c->f_lo, c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, T, r, c->p.n_cut, c->mc, c->kc, c->cur_flags,
+                acc_i, acc_j);
     }
     c->launches += last;
 }
@@ -234,19 +246,18 @@ template <int NC>
 void launch_pair_mixed_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles, c->n_chunks);
-    pair_mixed_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->n_pad, c->n_tiles,
-                                                       c->tiles_per_chunk, c->p.n_cut, c->mc,
-                                                       c->kc.halfL, c->flags, c->part);
+    pair_mixed_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->xy, c->zm, c->hs, c->tile_hmax,
+                                                       c->n_pad, c->n_tiles, c->tiles_per_chunk, c->p.n_cut,
+                                                       c->mc, c->kc, c->cur_flags, c->part);
 }
 
 template <int NC>
 void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
     dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
-    pair_mixed_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->tile_hmax, c->n_pad,
-                                                           c->n_tiles, c->sym_tiles_per_chunk,
-                                                           c->p.n_cut, c->mc, c->kc.halfL, c->flags,
-                                                           c->part);
+    pair_mixed_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->xy, c->zm, c->hs, c->tile_hmax,
+                                                           c->n_pad, c->n_tiles, c->sym_tiles_per_chunk,
+                                                           c->p.n_cut, c->mc, c->kc, c->cur_flags, c->part);
 }
 
 // EWALD_TABLE + DETERMINISTIC: one launch per round (pair_table_round.cuh).
@@ -297,7 +308,7 @@ void name_pair_kernel(steps_cyl_ctx *c)
         else snprintf(o, cap, "pair_table_%s_kernel<%d,%s>", det ? "round" : "sym", ip, c->d_table_f32 ? "16,true" : "4,false");
     } else if (ord) {
         if (mixed) snprintf(o, cap, "pair_mixed_kernel<%d>", nc);
-        else snprintf(o, cap, "pair_fp64_kernel<%d,0>", nc);
+        else snprintf(o, cap, "pair_fp64_kernel<%d>", nc);
     } else if (det) {
         snprintf(o, cap, "pair_%s_round_kernel<%d,%s>", mixed ? "mixed" : "fp64", nc, c->round_split > 1 ? "true" : "false");
     } else if (mixed) {
@@ -369,55 +380,229 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
         else if (c->use_rounds) launch_pair_rounds_nc<0>(c, s);
         else launch_pair_fp64_nc<0>(c, s);
     }
-    // general path: a no-op unless 2 max(h) > L/2
-    dim3 grid(c->n_tiles, c->n_chunks);
-    pair_fp64_kernel<0, 1><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles,
-                                                        c->tiles_per_chunk, c->p.n_cut, c->kc,
-                                                        c->flags, c->part);
-    c->launches += 2;
+    c->launches += 1;
 }
 
-int enqueue_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z,
-                  const double *m, const double *h, double *gx, double *gy, double *gz,
-                  cudaStream_t s)
+BgParams bg_params(const steps_cyl_ctx *c)
 {
-    const int tb = 256;
-    CK(cudaMemsetAsync(ctx->flags, 0, sizeof(DevFlags), s));
-    pack_kernel<<<ctx->n_tiles, PAIR_THREADS, 0, s>>>(x, y, z, m, h, ctx->n, ctx->n_pad, ctx->p.Lz,
-                                                     ctx->xy, ctx->zm, ctx->hs, ctx->f_hi, ctx->f_lo,
-                                                     ctx->tile_hmax, ctx->flags);
+    BgParams b;
+    b.R = c->p.R_sim;
+    b.Lhalf = (double)c->p.n_cut * c->p.Lz;
+    b.G = c->p.G;
+    b.rho0 = c->p.rho0;
+    b.infinite = c->p.background == STEPS_BG_INFINITE;
+    b.n_nodes = c->n_nodes;
+    b.nodes = c->nodes;
+    return b;
+}
+
+// Eq. 9 per particle is a 361-node quadrature: below this n one warp takes a particle (see aux_kernels.cuh)
+bool bg_warp_per_particle(const steps_cyl_ctx *c)
+{
+    return c->p.rho0 != 0.0 && c->p.background == STEPS_BG_FINITE && c->n <= 256 * 1024;
+}
+
+// One force evaluation = three launches: prestep (pack), the all-pairs kernel, poststep (reduction).  Inside a KDK
+// step (kick != nullptr) the first carries b(x_n), kick 1 and the drift, the last b(x_n+1) and kick 2.
+struct KdkArgs { double *vx, *vy, *vz; KickParams k1, k2; };
+
+// Argument blocks of the two O(N) kernels, in parameter order (launched through cudaLaunchKernel so that the same
+// blocks can re-parameterise the nodes of a captured graph, STEPS_FLAG_GRAPH).
+struct PreVals {
+    double *x, *y, *z, *vx, *vy, *vz;
+    const double *gx, *gy, *gz, *m, *h;
+    int n, n_pad;
+    double L;
+    BgParams bg;
+    KickParams kp;
+    double2 *xy, *zm;
+    double *hs;
+    float4 *f_hi, *f_lo;
+    double *tile_hmax;
+    DevFlags *fl;
+    int *sticky;
+    double *part;
+    int zero_rows;
+    void *args[26];
+    void bind()
+    {
+        void *a[26] = {&x, &y, &z, &vx, &vy, &vz, &gx, &gy, &gz, &m, &h, &n, &n_pad, &L, &bg, &kp, &xy, &zm, &hs,
+                       &f_hi, &f_lo, &tile_hmax, &fl, &sticky, &part, &zero_rows};
+        std::memcpy(args, a, sizeof a);
+    }
+};
+struct PostVals {
+    const double *part;
+    int n, n_pad, n_slabs;
+    double G, L;
+    DevFlags *fl_next;
+    double *gx, *gy, *gz;
+    const double *x, *y;
+    double *vx, *vy, *vz;
+    BgParams bg;
+    KickParams kp;
+    void *args[17];
+    void bind()
+    {
+        void *a[17] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz, &bg, &kp};
+        std::memcpy(args, a, sizeof a);
+    }
+};
+
+const void *prestep_func(bool kick, bool wpp)
+{
+    if (!kick) return (const void *)prestep_kernel<1, false>;
+    return wpp ? (const void *)prestep_kernel<32, true> : (const void *)prestep_kernel<1, true>;
+}
+const void *poststep_func(bool kick, bool wpp)
+{
+    if (!kick) return (const void *)poststep_kernel<1, false>;
+    return wpp ? (const void *)poststep_kernel<32, true> : (const void *)poststep_kernel<1, true>;
+}
+
+struct ForceArgs {
+    double *x, *y, *z;
+    const double *m, *h;
+    double *gx, *gy, *gz;
+    const KdkArgs *kick;
+};
+
+void fill_vals(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, PreVals &pre, PostVals &post)
+{
+    const KdkArgs *kick = f.kick;
+    const KickParams none = {0.0, 0.0, 0.0};
+    pre.x = f.x; pre.y = f.y; pre.z = f.z;
+    pre.vx = kick ? kick->vx : nullptr; pre.vy = kick ? kick->vy : nullptr; pre.vz = kick ? kick->vz : nullptr;
+    pre.gx = f.gx; pre.gy = f.gy; pre.gz = f.gz; pre.m = f.m; pre.h = f.h;
+    pre.n = ctx->n; pre.n_pad = ctx->n_pad; pre.L = ctx->p.Lz;
+    pre.bg = bg_params(ctx);
+    pre.kp = kick ? kick->k1 : none;
+    pre.xy = ctx->xy; pre.zm = ctx->zm; pre.hs = ctx->hs; pre.f_hi = ctx->f_hi; pre.f_lo = ctx->f_lo;
+    pre.tile_hmax = ctx->tile_hmax;
+    pre.fl = ctx->flags + (parity & 1u);
+    pre.sticky = ctx->bad_h_sticky;
+    pre.part = ctx->part;
+    // accumulator rows the pair kernel adds into (the ordered kernels overwrite theirs)
+    pre.zero_rows = ctx->use_sym ? 4 : (ctx->use_rounds ? 4 * (ctx->round_split + 1) : 0);
+    post.part = ctx->part; post.n = ctx->n; post.n_pad = ctx->n_pad;
+    post.n_slabs = ctx->use_sym ? 1 : (ctx->use_rounds ? ctx->round_split + 1 : ctx->n_chunks);
+    post.G = ctx->p.G; post.L = ctx->p.Lz;
+    post.fl_next = ctx->flags + ((parity + 1u) & 1u);
+    post.gx = f.gx; post.gy = f.gy; post.gz = f.gz; post.x = f.x; post.y = f.y;
+    post.vx = pre.vx; post.vy = pre.vy; post.vz = pre.vz;
+    post.bg = pre.bg;
+    post.kp = kick ? kick->k2 : none;
+}
+
+int enqueue_force_plain(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, bool timed, cudaStream_t s)
+{
+    PreVals pre;
+    PostVals post;
+    fill_vals(ctx, f, parity, pre, post);
+    pre.bind();
+    post.bind();
+    const bool wpp = bg_warp_per_particle(ctx), kick = f.kick != nullptr;
+    const dim3 grid(ctx->n_tiles), block(kick && wpp ? 1024 : PAIR_THREADS);
+    ctx->cur_flags = pre.fl;
+    CK(cudaLaunchKernel(prestep_func(kick, wpp), grid, block, pre.args, 0, s));
     ctx->launches += 1;
-    CK(cudaEventRecord(ctx->ev0, s));
-    if (ctx->use_sym)      // the symmetric kernels accumulate with atomics into part[0..4 n_pad)
-        CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * sizeof(double), s));
-    if (ctx->use_rounds)   // target-side sums in slab 0, source-side sums in slab 1 (its 4th row stays 0)
-        CK(cudaMemsetAsync(ctx->part, 0, 4 * (size_t)ctx->n_pad * (ctx->round_split + 1) * sizeof(double), s));
+    if (timed) CK(cudaEventRecord(ctx->ev0, s));
     launch_pair(ctx, s);
-    CK(cudaEventRecord(ctx->ev1, s));
-    ctx->ev_valid = true;
-    finalize_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->part, ctx->n, ctx->n_pad,
-                                                         ctx->use_sym ? 1 : (ctx->use_rounds ? ctx->round_split + 1 : ctx->n_chunks),
-                                                         ctx->table_mode ? (ctx->use_rounds ? 2 : 1) : ctx->n_chunks,
-                                                         ctx->kc.halfL, ctx->flags,
-                                                         ctx->p.G, ctx->p.Lz, gx, gy, gz);
+    if (timed) CK(cudaEventRecord(ctx->ev1, s));
+    ctx->ev_valid = timed;
+    CK(cudaLaunchKernel(poststep_func(kick, wpp), grid, block, post.args, 0, s));
     ctx->launches += 1;
     CK(cudaGetLastError());
     return STEPS_OK;
+}
+
+// STEPS_FLAG_GRAPH: the evaluation captured once per (flag-block parity, pointer set) as a CUDA graph; later calls
+// with the same pointers re-parameterise the two O(N) nodes (the kick scalars change every step) and replay it --
+// one launch per step instead of three.  The all-pairs kernel is not timed in this mode (no event nodes).
+void drop_graph(GraphSlot &g)
+{
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g = GraphSlot();
+}
+
+int enqueue_force_graph(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, cudaStream_t s)
+{
+    GraphSlot &g = ctx->gslot[parity & 1u];
+    const void *key[11] = {f.x, f.y, f.z, f.m, f.h, f.gx, f.gy, f.gz, f.kick ? f.kick->vx : nullptr,
+                           f.kick ? f.kick->vy : nullptr, f.kick ? f.kick->vz : nullptr};
+    const bool wpp = bg_warp_per_particle(ctx), kick = f.kick != nullptr;
+    if (g.exec && std::memcmp(key, g.key, sizeof key) != 0) drop_graph(g);
+    if (!g.exec) {
+        const int64_t before = ctx->launches;
+        CK(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+        int rc = enqueue_force_plain(ctx, f, parity, false, s);
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamEndCapture(s, &graph);
+        if (rc != STEPS_OK || e != cudaSuccess) {
+            if (graph) cudaGraphDestroy(graph);
+            return rc != STEPS_OK ? rc : cuda_fail(ctx, e);
+        }
+        g.graph = graph;
+        g.n_kernels = (int)(ctx->launches - before);
+        ctx->launches = before;
+        size_t n_nodes = 0;
+        CK(cudaGraphGetNodes(graph, nullptr, &n_nodes));
+        std::vector<cudaGraphNode_t> nodes(n_nodes);
+        CK(cudaGraphGetNodes(graph, nodes.data(), &n_nodes));
+        for (cudaGraphNode_t nd : nodes) {
+            cudaGraphNodeType ty;
+            CK(cudaGraphNodeGetType(nd, &ty));
+            if (ty != cudaGraphNodeTypeKernel) continue;
+            cudaKernelNodeParams kp;
+            CK(cudaGraphKernelNodeGetParams(nd, &kp));
+            if (kp.func == prestep_func(kick, wpp)) g.pre = nd;
+            if (kp.func == poststep_func(kick, wpp)) g.post = nd;
+        }
+        if (!g.pre || !g.post) { drop_graph(g); return STEPS_ECUDA; }
+        CK(cudaGraphInstantiate(&g.exec, graph, 0));
+        std::memcpy(g.key, key, sizeof key);
+    } else {
+        PreVals pre;
+        PostVals post;
+        fill_vals(ctx, f, parity, pre, post);
+        pre.bind();
+        post.bind();
+        cudaKernelNodeParams kp = {};
+        kp.gridDim = dim3(ctx->n_tiles);
+        kp.blockDim = dim3(kick && wpp ? 1024 : PAIR_THREADS);
+        kp.func = const_cast<void *>(prestep_func(kick, wpp));
+        kp.kernelParams = pre.args;
+        CK(cudaGraphExecKernelNodeSetParams(g.exec, g.pre, &kp));
+        kp.func = const_cast<void *>(poststep_func(kick, wpp));
+        kp.kernelParams = post.args;
+        CK(cudaGraphExecKernelNodeSetParams(g.exec, g.post, &kp));
+    }
+    CK(cudaGraphLaunch(g.exec, s));
+    ctx->launches += g.n_kernels;
+    ctx->ev_valid = false;
+    return STEPS_OK;
+}
+
+int enqueue_force(steps_cyl_ctx *ctx, double *x, double *y, double *z, const double *m, const double *h,
+                  double *gx, double *gy, double *gz, const KdkArgs *kick, cudaStream_t s)
+{
+    const ForceArgs f = {x, y, z, m, h, gx, gy, gz, kick};
+    const unsigned parity = ctx->eval_count & 1u;      // which of the two flag blocks this evaluation uses
+    ctx->eval_count += 1;
+    if (ctx->p.flags & STEPS_FLAG_GRAPH) return enqueue_force_graph(ctx, f, parity, s);
+    return enqueue_force_plain(ctx, f, parity, true, s);
 }
 
 int enqueue_background(steps_cyl_ctx *ctx, const double *x, const double *y, double *bx, double *by,
                        cudaStream_t s)
 {
     const int tb = 128;
-    const bool infinite = ctx->p.background == STEPS_BG_INFINITE;
-    if (!infinite && ctx->n <= 256 * 1024)       // one warp per particle: see background_kernel
-        background_kernel<32><<<(ctx->n * 32 + tb - 1) / tb, tb, 0, s>>>(
-            x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0, 0,
-            ctx->nodes, ctx->n_nodes, bx, by);
+    const BgParams bg = bg_params(ctx);
+    if (bg_warp_per_particle(ctx))
+        background_kernel<32><<<(ctx->n * 32 + tb - 1) / tb, tb, 0, s>>>(x, y, ctx->n, bg, bx, by);
     else
-        background_kernel<1><<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(
-            x, y, ctx->n, ctx->p.R_sim, (double)ctx->p.n_cut * ctx->p.Lz, ctx->p.G, ctx->p.rho0, infinite,
-            ctx->nodes, ctx->n_nodes, bx, by);
+        background_kernel<1><<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(x, y, ctx->n, bg, bx, by);
     ctx->launches += 1;
     CK(cudaGetLastError());
     return STEPS_OK;
@@ -439,7 +624,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         return STEPS_EINVAL;
     if (p->precision != STEPS_PREC_FP64 && p->precision != STEPS_PREC_MIXED) return STEPS_EINVAL;
     if (p->background != STEPS_BG_FINITE && p->background != STEPS_BG_INFINITE) return STEPS_EINVAL;
-    if ((p->flags & ~(STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_FAR_ORDER2 | STEPS_FLAG_ORDERED_PAIRS)) != 0 ||
+    if ((p->flags & ~(STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_FAR_ORDER2 | STEPS_FLAG_ORDERED_PAIRS | STEPS_FLAG_GRAPH)) != 0 ||
         p->device < 0)
         return STEPS_EINVAL;
     if (!std::isfinite(p->rho0) || !std::isfinite(p->R_sim)) return STEPS_EINVAL;
@@ -527,9 +712,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
     A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 5)));
-    A(dev_alloc(&ctx->bx, np));
-    A(dev_alloc(&ctx->by, np));
-    A(dev_alloc(&ctx->flags, 1));
+    A(dev_alloc(&ctx->flags, 3));                   // two alternating blocks + the sticky h <= 0 word
     A(dev_alloc(&ctx->peak_out, 1));
     A(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
     A(cudaEventCreate(&ctx->ev0));
@@ -583,8 +766,10 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         ctx->tc.inv_dz = (double)(pp.tab_nz - 1) / (0.5 * pp.Lz);
         ctx->tc.two_over_L = 2.0 / pp.Lz;
     }
-    A(cudaMemset(ctx->flags, 0, sizeof(DevFlags)));
+    A(cudaMemset(ctx->flags, 0, 3 * sizeof(DevFlags)));
     if (rc != STEPS_OK) return fail(rc);
+    ctx->bad_h_sticky = reinterpret_cast<int *>(ctx->flags + 2);
+    ctx->cur_flags = ctx->flags;
     name_pair_kernel(ctx);
     *out = ctx;
     return STEPS_OK;
@@ -593,8 +778,12 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
 void steps_cyl_destroy(steps_cyl_ctx *c)
 {
     if (!c) return;
+    for (GraphSlot &g : c->gslot) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (g.graph) cudaGraphDestroy(g.graph);
+    }
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->bx); cudaFree(c->by); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
+    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -608,7 +797,8 @@ int steps_cyl_accel(steps_cyl_ctx *ctx, const double *x, const double *y, const 
 {
     if (!ctx || !x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
     ON_DEVICE(ctx);
-    return enqueue_accel(ctx, x, y, z, m, h, gx, gy, gz, (cudaStream_t)cuda_stream);
+    return enqueue_force(ctx, const_cast<double *>(x), const_cast<double *>(y), const_cast<double *>(z), m, h,
+                         gx, gy, gz, nullptr, (cudaStream_t)cuda_stream);
 }
 
 int steps_cyl_check(steps_cyl_ctx *ctx, void *cuda_stream)
@@ -616,10 +806,11 @@ int steps_cyl_check(steps_cyl_ctx *ctx, void *cuda_stream)
     if (!ctx) return STEPS_EINVAL;
     ON_DEVICE(ctx);
     CK(cudaStreamSynchronize((cudaStream_t)cuda_stream));
-    DevFlags f;
-    CK(cudaMemcpy(&f, ctx->flags, sizeof f, cudaMemcpyDeviceToHost));
+    int bad = 0;
+    CK(cudaMemcpy(&bad, ctx->bad_h_sticky, sizeof bad, cudaMemcpyDeviceToHost));
+    if (bad) CK(cudaMemset(ctx->bad_h_sticky, 0, sizeof bad));          // reported once, then cleared
     CK(cudaGetLastError());
-    return f.bad_h ? STEPS_ESOFT : STEPS_OK;
+    return bad ? STEPS_ESOFT : STEPS_OK;
 }
 
 int steps_cyl_accel_host(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z,
@@ -636,7 +827,7 @@ int steps_cyl_accel_host(steps_cyl_ctx *ctx, const double *x, const double *y, c
     double *d = ctx->host_io;
     const double *src[5] = {x, y, z, m, h};
     for (int k = 0; k < 5; ++k) CK(cudaMemcpyAsync(d + k * n, src[k], B, cudaMemcpyHostToDevice, s));
-    int rc = enqueue_accel(ctx, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d + 7 * n, s);
+    int rc = enqueue_force(ctx, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d + 7 * n, nullptr, s);
     if (rc != STEPS_OK) return rc;
     double *dst[3] = {gx, gy, gz};
     for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], d + (5 + k) * n, B, cudaMemcpyDeviceToHost, s));
@@ -659,24 +850,12 @@ int steps_cyl_kdk_step(steps_cyl_ctx *ctx, double *x, double *y, double *z, doub
     if (!ctx || !x || !y || !z || !vx || !vy || !vz || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
     if (!(a_n > 0.0) || !(a_np1 > 0.0) || !std::isfinite(dt)) return STEPS_EINVAL;
     ON_DEVICE(ctx);
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    const int tb = 256, nb = (ctx->n + tb - 1) / tb;
-    // b(x_n): the caller may have moved the particles since the last step, so it is recomputed
-    // (O(N), ~1e-3 of the pair sum).
-    int rc = enqueue_background(ctx, x, y, ctx->bx, ctx->by, s);
-    if (rc != STEPS_OK) return rc;
-    kick1_drift_kernel<<<nb, tb, 0, s>>>(x, y, z, vx, vy, vz, gx, gy, gz, ctx->bx, ctx->by, ctx->n,
-                                         1.0 / (a_n * a_n * a_n), H_n, dt, ctx->p.Lz);
-    ctx->launches += 1;
-    rc = enqueue_accel(ctx, x, y, z, m, h, gx, gy, gz, s);
-    if (rc != STEPS_OK) return rc;
-    rc = enqueue_background(ctx, x, y, ctx->bx, ctx->by, s);
-    if (rc != STEPS_OK) return rc;
-    kick2_kernel<<<nb, tb, 0, s>>>(vx, vy, vz, gx, gy, gz, ctx->bx, ctx->by, ctx->n,
-                                   1.0 / (a_np1 * a_np1 * a_np1), H_np1, dt);
-    ctx->launches += 1;
-    CK(cudaGetLastError());
-    return STEPS_OK;
+    KdkArgs k;
+    k.vx = vx; k.vy = vy; k.vz = vz;
+    k.k1 = {1.0 / (a_n * a_n * a_n), H_n, dt};
+    k.k2 = {1.0 / (a_np1 * a_np1 * a_np1), H_np1, dt};
+    // b(x_n) is recomputed inside prestep_kernel: the caller may have moved the particles since the last step
+    return enqueue_force(ctx, x, y, z, m, h, gx, gy, gz, &k, (cudaStream_t)cuda_stream);
 }
 
 int steps_cyl_kdk_step_host(steps_cyl_ctx *ctx, double *x, double *y, double *z, double *vx,

@@ -99,7 +99,12 @@ def _base(op):
 
 
 def analyse(ins):
-    """Pair loop of one kernel: (start, end, mainline Counter, skippable Counter, nested) or None."""
+    """Pair loop of one kernel: (start, end, mainline Counter, slow-path Counter, nested) or None."""
+    # out-of-line device functions (the noinline spline, the general-path bodies) are listed after the kernel's
+    # own code, from the lowest CALL target on: the pair loop is looked for in the kernel's own code only
+    calls = [int(m.group(1), 16) for _, _, t in ins if t.startswith("CALL") for m in [re.search(r"0x([0-9a-f]+)", t)] if m]
+    if calls:
+        ins = [i for i in ins if i[0] < min(calls)]
     loops = []
     for a, pred, t in ins:
         m = _BRA.search(t)

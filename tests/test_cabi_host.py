@@ -48,7 +48,7 @@ def test_init_rejects_bad_arguments(lib):
     good = dict(n=16, Lz=100.0, G=1.0, periodic_mode=0, n_cut=5, precision=0, background=0,
                 R_sim=0.0, rho0=0.0, device=0, flags=0)
     for bad in (dict(n=0), dict(Lz=0.0), dict(Lz=-1.0), dict(n_cut=0), dict(precision=7),
-                dict(background=3), dict(periodic_mode=9), dict(flags=8), dict(device=-1),
+                dict(background=3), dict(periodic_mode=9), dict(flags=16), dict(device=-1),
                 dict(rho0=1.0, R_sim=0.0), dict(n=2 ** 31), dict(n=64 * 65535 * 128 + 1)):
         p = b.Params(**{**good, **bad})
         assert lib.steps_cyl_init(C.byref(p), C.byref(ctx)) == b.STEPS_EINVAL, bad

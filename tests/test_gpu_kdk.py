@@ -206,3 +206,72 @@ def test_glass_making_with_repulsive_gravity(torch_cuda):
     ctx.close()
     assert 0.10 < r0 < 0.25 and r1 < 0.75 * r0, (r0, r1)
     assert all(math.isfinite(sp) for sp in speeds) and speeds[1] < speeds[0]
+
+
+def test_step_is_three_launches_and_graph_replay_matches(torch_cuda, oracle):
+    """A KDK step is three launches (prestep: b + kick + drift + pack; the all-pairs kernel; poststep: reduction +
+    b + kick).  STEPS_FLAG_GRAPH replays the same three kernels as one captured CUDA graph whose two O(N) nodes are
+    re-parameterised every step: with the deterministic kernels the trajectories are bit-identical, and a change of
+    the caller's pointers re-captures."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(3, n=3000)
+    c = w.cosmo
+    names = ("x", "y", "z", "vx", "vy", "vz", "m", "h")
+
+    def run(flags, swap_at=None):
+        ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=w.n_cut, R_sim=w.R_sim, rho0=w.rho0, flags=flags)
+        dev = {k: _dev(torch, getattr(w, k)) for k in names}
+        g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+        a = c["a_init"]
+        _, H = b.friedmann_step(a, 0.0, c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+        per_step = []
+        for s in range(6):
+            if s == swap_at:                      # the caller moves its arrays: new pointers, same values
+                dev = {k: v.clone() for k, v in dev.items()}
+                g = [t.clone() for t in g]
+            a1, H1 = b.friedmann_step(a, c["dt"], c["H0"], c["Om"], c["Or"], c["Ok"], c["OL"])
+            n0 = ctx.launch_count()
+            ctx.kdk_step(*[dev[k] for k in names], *g, a, H, a1, H1, c["dt"])
+            per_step.append(ctx.launch_count() - n0)
+            a, H = a1, H1
+        ctx.check()
+        out = [dev[k].cpu().numpy() for k in names[:6]] + [t.cpu().numpy() for t in g]
+        ctx.close()
+        return out, per_step
+
+    ref, launches = run(0)
+    assert launches == [3] * 6
+    got, launches = run(b.FLAG_GRAPH)
+    assert launches == [3] * 6                    # kernels inside the replayed graph
+    for p, q in zip(got, ref):                    # atomics: same terms, summation order free
+        assert np.abs(p - q).max() <= 1e-11 * np.abs(q).max()
+    det, _ = run(b.FLAG_DETERMINISTIC)
+    for flags, swap in ((b.FLAG_DETERMINISTIC | b.FLAG_GRAPH, None), (b.FLAG_DETERMINISTIC | b.FLAG_GRAPH, 3)):
+        got, _ = run(flags, swap)
+        for p, q in zip(got, det):
+            assert np.array_equal(p, q)
+
+
+def test_accel_with_graph_flag(torch_cuda, oracle):
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(1, n=2500, seed=13)
+    ref = np.stack(oracle.accel(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, 5), 1)
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=5, flags=b.FLAG_GRAPH)
+    dev = [_dev(torch, a) for a in (w.x, w.y, w.z, w.m, w.h)]
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    for _ in range(3):                            # capture (both flag-block parities), then replay
+        for t in g:
+            t.fill_(float("nan"))
+        ctx.accel(*dev, *g)
+        ctx.check()
+        got = np.stack([t.cpu().numpy() for t in g], 1)
+        e = np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)
+        assert e.max() <= 1e-10
+    with pytest.raises(b.StepsError):
+        ctx.last_pair_kernel_ms()                 # the kernel is not timed on its own inside a graph
+    ctx.close()

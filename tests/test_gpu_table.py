@@ -282,3 +282,26 @@ def test_table_mode_bench_size_sampled_targets(torch_cuda, oracle, variant):
         assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN, (e.max(), np.median(e))
     for c in g:
         assert abs(np.sum(w.m * c)) <= (1e-11 if variant != "mixed" else 1e-5) * np.sum(w.m * np.abs(c))
+
+
+def test_two_live_contexts_with_different_table_sizes(torch_cuda, oracle):
+    """The dynamic shared-memory limit of the table kernels is a per-function, process-wide setting: a second
+    context with a smaller float table must not lower it under the first one's feet."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(0, n=1500, seed=4)
+    dev = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.x, w.y, w.z, w.m, w.h)]
+    shapes = [(144, 128, 500.0), (40, 33, 150.0)]
+    ctxs = [b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, periodic_mode=b.PERIODIC_EWALD_TABLE, tab_fp32=1, tab_nrho=nr,
+                       tab_nz=nz, tab_rho_max=rm) for nr, nz, rm in shapes]        # big first, then small
+    for ctx, (nr, nz, rm) in zip(ctxs, shapes):
+        D32 = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, nr, nz, rm).astype(np.float32).astype(np.float64)
+        ref = oracle.accel_table(w.x, w.y, w.z, w.m, w.h, w.Lz, w.G, D32, rm, 0)
+        g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        ctx.accel(*dev, *g)
+        ctx.check()
+        e = rel_err([t.cpu().numpy() for t in g], ref)
+        assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN
+    for ctx in ctxs:
+        ctx.close()

@@ -29,7 +29,7 @@ def every_selectable_kernel():
         names += ["pair_fp64_sym_kernel<%d,%s>" % (nc, o2) for o2 in ("false", "true")]
         names += ["pair_fp64_round_kernel<%d,%s>" % (nc, sp) for sp in ("false", "true")]
         names += ["pair_mixed_round_kernel<%d,%s>" % (nc, sp) for sp in ("false", "true")]
-        names += ["pair_fp64_kernel<%d,0>" % nc, "pair_mixed_kernel<%d>" % nc, "pair_mixed_sym_kernel<%d>" % nc]
+        names += ["pair_fp64_kernel<%d>" % nc, "pair_mixed_kernel<%d>" % nc, "pair_mixed_sym_kernel<%d>" % nc]
     for ip, sched in itertools.product((0, 1), ("sym", "round")):       # CIC and TSC
         names += ["pair_table_%s_kernel<%d,4,false>" % (sched, ip), "pair_table_%s_kernel<%d,16,true>" % (sched, ip),
                   "pair_table_mixed_%s_kernel<%d>" % (sched, ip)]
@@ -62,7 +62,7 @@ def test_default_fp64_kernel_count(mix):
 
 def test_per_image_cost_from_unrolled_instances(mix):
     from paper_2602_20787_b200 import sassmix
-    for fam, lo, hi in (("pair_fp64_sym_kernel<%d,false>", 8.0, 10.5), ("pair_fp64_kernel<%d,0>", 17.0, 21.0)):
+    for fam, lo, hi in (("pair_fp64_sym_kernel<%d,false>", 8.0, 10.5), ("pair_fp64_kernel<%d>", 17.0, 21.0)):
         d = (mix["kernels"][fam % 8]["per_interaction"]["fp64_instr"]
              - mix["kernels"][fam % 7]["per_interaction"]["fp64_instr"])
         assert lo <= d <= hi, (fam, d)              # two more images per pair evaluation
