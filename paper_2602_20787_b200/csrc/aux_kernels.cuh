@@ -51,9 +51,11 @@ __device__ __forceinline__ double background_nodes(double rho, double R, double 
 // The O(N) work of a force evaluation / KDK step is two launches around the all-pairs kernel:
 //   prestep_kernel  : [b(x_n), kick 1, drift]  pack + wrap (a1), zero the accumulators, max(h), h <= 0
 //   poststep_kernel : partial-sum reduction (a5)  [b(x_n+1), kick 2]
-// (the bracketed parts only inside steps_cyl_kdk_step).  One CTA per 128-particle tile.  LANES = 32: the CTA
-// has 32 warps and the Eq. 9 quadrature of each particle is spread over the lanes of a warp (small n, where one
-// thread per particle would leave most SMs empty for the 361-node loop); LANES = 1: 128 threads, one per particle.
+// (the bracketed parts only inside steps_cyl_kdk_step).
+//   LANES = 1 : one thread per particle, one 128-thread CTA per tile;
+//   LANES = 32: one WARP per particle, 8 particles per 256-thread CTA -- the Eq. 9 quadrature (361 nodes, ~100 FP64
+//               instructions each) is then spread over the lanes and over every SM; with a thread per particle it would
+//               outlast the pair kernel at small n (n = 2048: 128 particles x 361 nodes on each of 16 SMs).
 struct BgParams {
     double R, Lhalf, G, rho0;
     int infinite;                    // Eq. 10 instead of Eq. 9
@@ -61,6 +63,11 @@ struct BgParams {
     const QuadNode *nodes;
 };
 struct KickParams { double inv_a3, H, dt; };
+
+template <int LANES> struct OnStep {
+    static constexpr int kParticlesPerBlock = (LANES == 32) ? 8 : PAIR_THREADS;
+    static constexpr int kThreads = (LANES == 32) ? 256 : PAIR_THREADS;
+};
 
 // s with b = s (x, y): s = -F_h(rho)/rho (Eq. 11 subtracts F_h < 0: outward push); 0 when disabled or on the axis.
 // LANES == 32: called by a whole warp for ONE particle, every lane returns the sum.
@@ -84,33 +91,19 @@ __device__ __forceinline__ double background_scale(double xv, double yv, const B
     return -Fh / rho;
 }
 
-// Background scale of the tile's 128 particles into s_bg[128] (LANES == 32) or the caller's register.
-template <int LANES>
-__device__ __forceinline__ double tile_background(const double *__restrict__ x, const double *__restrict__ y,
-                                                  int tile, int n, const BgParams &bg, double *s_bg)
+__device__ __forceinline__ void atomic_max_positive(double *addr, double v)      // v > 0: bit patterns order like values
 {
-    if (LANES == 1) {
-        const int i = tile * PAIR_THREADS + threadIdx.x;
-        return (i < n) ? background_scale<1>(x[i], y[i], bg, 0) : 0.0;
-    }
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#pragma unroll 1
-    for (int q = 0; q < PAIR_THREADS / 32; ++q) {                      // 32 warps x 4 particles
-        const int p = w * (PAIR_THREADS / 32) + q, i = tile * PAIR_THREADS + p;
-        const double sv = (i < n) ? background_scale<32>(x[i], y[i], bg, lane) : 0.0;      // i is warp-uniform
-        if (lane == 0) s_bg[p] = sv;
-    }
-    __syncthreads();
-    return (threadIdx.x < PAIR_THREADS) ? s_bg[threadIdx.x] : 0.0;
+    atomicMax(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)__double_as_longlong(v));
 }
 
 // a1 (+ a6, a7 first half when KICK).  KICK (reading S4):
 //   v <- v + (dt/2)[(g + b)/a_n^3 - 2 H_n v];  x <- x + v dt;  z reduced to [0, L)
 // then, for the positions the force is wanted at: SoA -> packed, padded source arrays (massless far-away dummies
-// beyond n), float hi/lo splits for the mixed kernels, per-tile max h (bounds h_i + h_j in the spline pre-test),
-// global max h and the h <= 0 flag, and zeroed accumulator rows part[0 .. zero_rows) x [n_pad].
+// beyond n), float hi/lo splits for the mixed kernels, per-tile max h (bounds h_i + h_j in the spline pre-test;
+// tile_hmax is zero on entry -- poststep_kernel clears it), global max h and the h <= 0 flag, and zeroed
+// accumulator rows part[0 .. zero_rows) x [n_pad].   grid = n_pad / particles per block.
 template <int LANES, bool KICK>
-__global__ void __launch_bounds__(LANES == 32 ? 1024 : PAIR_THREADS)
+__global__ void __launch_bounds__(OnStep<LANES>::kThreads)
 prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restrict__ z,
                double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
                const double *__restrict__ gx, const double *__restrict__ gy, const double *__restrict__ gz,
@@ -121,15 +114,16 @@ prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restric
                DevFlags *__restrict__ flags, int *__restrict__ bad_h_sticky,
                double *__restrict__ part, int zero_rows)
 {
-    __shared__ double s_bg[PAIR_THREADS];
-    __shared__ double s_max[PAIR_THREADS / 32];
-    double sb = 0.0;
-    if (KICK) sb = tile_background<LANES>(x, y, blockIdx.x, n, bg, s_bg);
-    if (threadIdx.x >= PAIR_THREADS) return;
-    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const int i = (LANES == 32) ? blockIdx.x * OnStep<LANES>::kParticlesPerBlock + (threadIdx.x >> 5)
+                                : blockIdx.x * PAIR_THREADS + threadIdx.x;           // < n_pad
     double xv, yv, zv, mv, hv;
     if (i < n) {
-        xv = x[i]; yv = y[i]; zv = z[i]; mv = m[i]; hv = h[i];
+        xv = x[i]; yv = y[i];
+        double sb = 0.0;
+        if (KICK) sb = background_scale<LANES>(xv, yv, bg, lane);
+        if (LANES == 32 && lane != 0) return;
+        zv = z[i]; mv = m[i]; hv = h[i];
         if (KICK) {
             const double hdt = 0.5 * kp.dt;
             double ux = vx[i], uy = vy[i], uz = vz[i];
@@ -145,25 +139,31 @@ prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restric
             zv = wrap_z(zv, L);
         }
         if (!(hv > 0.0)) { atomicOr(&flags->bad_h, 1); atomicOr(bad_h_sticky, 1); }
-        else atomicMax(&flags->hmax_bits, (unsigned long long)__double_as_longlong(hv));
     } else {                   // massless dummy far outside any particle load
+        if (LANES == 32 && lane != 0) return;
         xv = 1.0e60; yv = 1.0e60; zv = 0.0; mv = 0.0; hv = 1.0;
     }
     xy[i] = make_double2(xv, yv);
     zm[i] = make_double2(zv, mv);
     hs[i] = hv;
     for (int r = 0; r < zero_rows; ++r) part[(size_t)r * n_pad + i] = 0.0;
-    {   // max h of the tile (dummies count as 0)
-        double hm = (i < n && hv > 0.0) ? hv : 0.0;
+    const double hm = (i < n && hv > 0.0) ? hv : 0.0;         // dummies count as 0
+    if (LANES == 32) {
+        if (hm > 0.0) {
+            atomic_max_positive(tile_hmax + i / PAIR_THREADS, hm);
+            atomicMax(&flags->hmax_bits, (unsigned long long)__double_as_longlong(hm));
+        }
+    } else {                   // the CTA is the tile: shuffle / shared-memory reduction, one store
+        __shared__ double s_max[PAIR_THREADS / 32];
+        double t = hm;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) hm = fmax(hm, __shfl_xor_sync(0xffffffffu, hm, o));
-        if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = hm;
-        // only the first four warps are here: a named barrier over them (bar 1), not __syncthreads
-        asm volatile("bar.sync 1, %0;" ::"n"(PAIR_THREADS));
+        for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_xor_sync(0xffffffffu, t, o));
+        if (lane == 0) s_max[threadIdx.x >> 5] = t;
+        __syncthreads();
         if (threadIdx.x == 0) {
-            double t = s_max[0];
             for (int wq = 1; wq < PAIR_THREADS / 32; ++wq) t = fmax(t, s_max[wq]);
             tile_hmax[blockIdx.x] = t;
+            if (t > 0.0) atomicMax(&flags->hmax_bits, (unsigned long long)__double_as_longlong(t));
         }
     }
     if (f_hi) {
@@ -180,23 +180,29 @@ prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restric
 
 // a5 (+ a6, a7 second half when KICK): g = -G (A_x, A_y, A_z1 - L A_z2), the partial sums added over the n_slabs
 // slabs the pair kernel wrote, in fixed order; KICK:  v <- [v + (dt/2)(g' + b')/a_{n+1}^3] / (1 + H_{n+1} dt).
-// Also clears the flag block the NEXT call's prestep will use (flags alternate between two blocks, so that no
-// memset sits between the launches).
+// Also clears what the NEXT evaluation's prestep accumulates into with atomics: the other flag block (flags
+// alternate between two blocks, so that no memset sits between the launches) and tile_hmax.
 template <int LANES, bool KICK>
-__global__ void __launch_bounds__(LANES == 32 ? 1024 : PAIR_THREADS)
+__global__ void __launch_bounds__(OnStep<LANES>::kThreads)
 poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, double G, double L,
-                DevFlags *__restrict__ flags_next,
+                DevFlags *__restrict__ flags_next, double *__restrict__ tile_hmax,
                 double *__restrict__ gx, double *__restrict__ gy, double *__restrict__ gz,
                 const double *__restrict__ x, const double *__restrict__ y,
                 double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
                 BgParams bg, KickParams kp)
 {
-    __shared__ double s_bg[PAIR_THREADS];
+    const int lane = threadIdx.x & 31;
+    const int i = (LANES == 32) ? blockIdx.x * OnStep<LANES>::kParticlesPerBlock + (threadIdx.x >> 5)
+                                : blockIdx.x * PAIR_THREADS + threadIdx.x;           // < n_pad
     if (blockIdx.x == 0 && threadIdx.x == 0) { flags_next->hmax_bits = 0ull; flags_next->bad_h = 0; }
-    double sb = 0.0;
-    if (KICK) sb = tile_background<LANES>(x, y, blockIdx.x, n, bg, s_bg);
-    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
-    if (threadIdx.x >= PAIR_THREADS || i >= n) return;
+    if ((i % PAIR_THREADS) == 0 && lane == 0) tile_hmax[i / PAIR_THREADS] = 0.0;
+    if (i >= n) return;
+    double sb = 0.0, xv = 0.0, yv = 0.0;
+    if (KICK) {
+        xv = x[i]; yv = y[i];
+        sb = background_scale<LANES>(xv, yv, bg, lane);
+    }
+    if (LANES == 32 && lane != 0) return;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     for (int c = 0; c < n_slabs; ++c) {
         const double *p = part + (size_t)c * 4 * n_pad + i;
@@ -209,8 +215,8 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
     gx[i] = g0; gy[i] = g1; gz[i] = g2;
     if (KICK) {
         const double hdt = 0.5 * kp.dt, den = 1.0 + kp.H * kp.dt;
-        vx[i] = (vx[i] + hdt * (g0 + sb * x[i]) * kp.inv_a3) / den;
-        vy[i] = (vy[i] + hdt * (g1 + sb * y[i]) * kp.inv_a3) / den;
+        vx[i] = (vx[i] + hdt * (g0 + sb * xv) * kp.inv_a3) / den;
+        vy[i] = (vy[i] + hdt * (g1 + sb * yv) * kp.inv_a3) / den;
         vz[i] = (vz[i] + hdt * g2 * kp.inv_a3) / den;
     }
 }

@@ -436,15 +436,17 @@ struct PostVals {
     int n, n_pad, n_slabs;
     double G, L;
     DevFlags *fl_next;
+    double *tile_hmax;
     double *gx, *gy, *gz;
     const double *x, *y;
     double *vx, *vy, *vz;
     BgParams bg;
     KickParams kp;
-    void *args[17];
+    void *args[18];
     void bind()
     {
-        void *a[17] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz, &bg, &kp};
+        void *a[18] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &tile_hmax, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz,
+                       &bg, &kp};
         std::memcpy(args, a, sizeof a);
     }
 };
@@ -458,6 +460,16 @@ const void *poststep_func(bool kick, bool wpp)
 {
     if (!kick) return (const void *)poststep_kernel<1, false>;
     return wpp ? (const void *)poststep_kernel<32, true> : (const void *)poststep_kernel<1, true>;
+}
+
+// launch geometry of prestep / poststep (aux_kernels.cuh: OnStep<LANES>)
+int onstep_block(const steps_cyl_ctx *c, bool kick)
+{
+    return (kick && bg_warp_per_particle(c)) ? OnStep<32>::kThreads : OnStep<1>::kThreads;
+}
+int onstep_grid(const steps_cyl_ctx *c, bool kick)
+{
+    return c->n_pad / ((kick && bg_warp_per_particle(c)) ? OnStep<32>::kParticlesPerBlock : OnStep<1>::kParticlesPerBlock);
 }
 
 struct ForceArgs {
@@ -488,6 +500,7 @@ void fill_vals(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, PreVals 
     post.n_slabs = ctx->use_sym ? 1 : (ctx->use_rounds ? ctx->round_split + 1 : ctx->n_chunks);
     post.G = ctx->p.G; post.L = ctx->p.Lz;
     post.fl_next = ctx->flags + ((parity + 1u) & 1u);
+    post.tile_hmax = ctx->tile_hmax;
     post.gx = f.gx; post.gy = f.gy; post.gz = f.gz; post.x = f.x; post.y = f.y;
     post.vx = pre.vx; post.vy = pre.vy; post.vz = pre.vz;
     post.bg = pre.bg;
@@ -502,7 +515,7 @@ int enqueue_force_plain(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity,
     pre.bind();
     post.bind();
     const bool wpp = bg_warp_per_particle(ctx), kick = f.kick != nullptr;
-    const dim3 grid(ctx->n_tiles), block(kick && wpp ? 1024 : PAIR_THREADS);
+    const dim3 grid(onstep_grid(ctx, kick)), block(onstep_block(ctx, kick));
     ctx->cur_flags = pre.fl;
     CK(cudaLaunchKernel(prestep_func(kick, wpp), grid, block, pre.args, 0, s));
     ctx->launches += 1;
@@ -535,10 +548,13 @@ int enqueue_force_graph(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity,
     if (g.exec && std::memcmp(key, g.key, sizeof key) != 0) drop_graph(g);
     if (!g.exec) {
         const int64_t before = ctx->launches;
-        CK(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
-        int rc = enqueue_force_plain(ctx, f, parity, false, s);
+        // captured on the context's own stream (the caller's may be the legacy default stream, which cannot
+        // capture); the graph is launched on the caller's stream
+        cudaStream_t cs = ctx->own_stream;
+        CK(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+        int rc = enqueue_force_plain(ctx, f, parity, false, cs);
         cudaGraph_t graph = nullptr;
-        cudaError_t e = cudaStreamEndCapture(s, &graph);
+        cudaError_t e = cudaStreamEndCapture(cs, &graph);
         if (rc != STEPS_OK || e != cudaSuccess) {
             if (graph) cudaGraphDestroy(graph);
             return rc != STEPS_OK ? rc : cuda_fail(ctx, e);
@@ -569,8 +585,8 @@ int enqueue_force_graph(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity,
         pre.bind();
         post.bind();
         cudaKernelNodeParams kp = {};
-        kp.gridDim = dim3(ctx->n_tiles);
-        kp.blockDim = dim3(kick && wpp ? 1024 : PAIR_THREADS);
+        kp.gridDim = dim3(onstep_grid(ctx, kick));
+        kp.blockDim = dim3(onstep_block(ctx, kick));
         kp.func = const_cast<void *>(prestep_func(kick, wpp));
         kp.kernelParams = pre.args;
         CK(cudaGraphExecKernelNodeSetParams(g.exec, g.pre, &kp));
@@ -709,6 +725,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->zm, np));
     A(dev_alloc(&ctx->hs, np));
     A(dev_alloc(&ctx->tile_hmax, (size_t)ctx->n_tiles));
+    if (rc == STEPS_OK) A(cudaMemset(ctx->tile_hmax, 0, (size_t)ctx->n_tiles * sizeof(double)));
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
     A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 5)));
