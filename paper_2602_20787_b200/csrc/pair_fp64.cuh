@@ -62,6 +62,9 @@ __device__ __forceinline__ double rsqrt_seed(double x)
 
 // (x)^(-3/2) for normal positive x, ~1.5 ulp.  Series remainder 35/16 e^3 < 2^-55 for |e| < 2^-19 (measured:
 // |e| <= 1.84e-6 = 2^-19.05 for the RSQ64H seed).
+// Operand forms matter on this pipe (measured, profiles/r2_fp64_pipe_microbench.md): an FP64 instruction with THREE
+// distinct register sources takes three issue cycles instead of two, so the last step is written c * (1 + e p)
+// (DFMA with an immediate addend, then DMUL) rather than fma(c e, p, c).
 __device__ __forceinline__ double inv_cube_sqrt(double x)
 {
     const double y0 = rsqrt_seed(x);
@@ -69,7 +72,8 @@ __device__ __forceinline__ double inv_cube_sqrt(double x)
     const double e  = fma(-x, y2, 1.0);
     const double c  = y2 * y0;
     const double p  = fma(1.875, e, 1.5);
-    return fma(c * e, p, c);
+    const double g  = fma(e, p, 1.0);
+    return c * g;
 }
 
 // The same with the series cut after the linear term, w = y0^3 (1 + d0 + 3e/2): 5 FP64 instructions.
@@ -193,50 +197,99 @@ __device__ __forceinline__ void image_sum(double rz, double q, double hi, double
     }
 }
 
-// Run-time N_cut (NC == 0) for R targets against the same source: the image loop is the OUTER loop and the
-// targets the inner one, so that one trip has 2 R independent rsqrt chains (per unroll step) in flight and reads the
-// per-image constants once.  Same arithmetic per pair as image_sum<0>; N_cut > MAX_NCUT_TABLE falls back to it.
-template <int R, bool O2>
-__device__ __forceinline__ void image_sum_rt(const double (&rz)[R], const double (&q)[R],
-                                             const double (&hi)[R], double hj, const int (&soft_hi)[R],
-                                             const PairConsts &k, int ncut_rt, double (&S)[R], double (&T)[R])
+// Image sums of R pairs that share the source (the ring kernels: R targets of a lane), written for |r_z|:
+//     S = sum_n w_n (as above),   Ta = sum_n n w_n evaluated at |r_z|  ( = sign(r_z) T ),
+// so that the end image always sits at n = +N_cut (an immediate instead of a copysign'd register) and
+// sum_n w_n (r_z - n L) = sign(r_z) (S |r_z| - L Ta).  arz = |r_z|, q = rho^2 + r_z^2.
+// The spline pre-test of the R pairs is ONE warp-level branch.  NC > 0: unrolled; NC == 0: run-time N_cut with the
+// image loop outside the targets (2 R independent rsqrt chains per trip, per-image constants read once).
+template <int NC, int R, bool O2>
+__device__ __forceinline__ void image_sums(const double (&arz)[R], const double (&q)[R],
+                                           const double (&hi)[R], double hj, const int (&soft_hi)[R],
+                                           const PairConsts &k, int ncut_rt, double (&S)[R], double (&Ta)[R])
 {
-    if (ncut_rt > MAX_NCUT_TABLE) {
-#pragma unroll
-        for (int r = 0; r < R; ++r) image_sum<0, O2>(rz[r], q[r], hi[r], hj, soft_hi[r], k, ncut_rt, S[r], T[r]);
-        return;
-    }
+    bool any_soft = false;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        double w0 = inv_cube_sqrt(q[r]);
-        if (hi32(q[r]) <= soft_hi[r]) {
-            const double hh = hi[r] + hj;
-            if (q[r] < hh * hh) w0 = spline_w(q[r], hh);
-        }
-        S[r] = w0;
-        T[r] = 0.0;
+        S[r] = inv_cube_sqrt(q[r]);                       // nearest image n = 0 (the only one the spline can touch)
+        any_soft |= hi32(q[r]) <= soft_hi[r];
     }
-#pragma unroll kRtUnroll
-    for (int n = 1; n < ncut_rt; ++n) {
-        const double c = k.c2nL[n], b = k.n2L2[n], d = k.dn[n];
+    if (any_soft) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const double B  = q[r] + b;
-            const double wp = inv_cube_sqrt_far<O2>(fma(-c, rz[r], B));
-            const double wm = inv_cube_sqrt_far<O2>(fma(c, rz[r], B));
-            S[r] += wp;
-            S[r] += wm;
-            T[r] = fma(d, wp - wm, T[r]);
+            const double hh = hi[r] + hj;
+            if (q[r] < hh * hh) S[r] = spline_w(q[r], hh);
         }
     }
-    const double ce = k.c2nL[ncut_rt], be = k.n2L2[ncut_rt], de = k.dn[ncut_rt];
+    if (NC > 0) {
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const bool rz_nonzero = ((hi32(rz[r]) & 0x7fffffff) | lo32(rz[r])) != 0;
-        double we = inv_cube_sqrt_far<O2>(fma(-ce, fabs(rz[r]), q[r] + be));
-        we = rz_nonzero ? we : 0.0;
-        S[r] += we;
-        T[r] = fma(copysign(de, rz[r]), we, T[r]);
+        for (int n = 1; n < NC; ++n) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double B  = q[r] + k.n2L2[n];
+                const double wp = inv_cube_sqrt_far<O2>(fma(-k.c2nL[n], arz[r], B));   // image +n: d = |rz| - nL
+                const double wm = inv_cube_sqrt_far<O2>(fma(k.c2nL[n], arz[r], B));    // image -n: d = |rz| + nL
+                S[r] = __dadd_rn(S[r], wp);          // not contracted with w = c g: that DFMA would have three register sources
+                S[r] = __dadd_rn(S[r], wm);
+                Ta[r] = (n == 1) ? (wp - wm) : fma((double)n, wp - wm, Ta[r]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            // end image n = +N_cut (absent when rz == 0): d = -(N L - |rz|)
+            double we = inv_cube_sqrt_far<O2>(fma(-k.c2nL[NC], arz[r], q[r] + k.n2L2[NC]));
+            we = ((hi32(arz[r]) & 0x7fffffff) | lo32(arz[r])) != 0 ? we : 0.0;
+            S[r] = __dadd_rn(S[r], we);
+            Ta[r] = (NC == 1) ? we : fma((double)NC, we, Ta[r]);
+        }
+    } else if (ncut_rt <= MAX_NCUT_TABLE) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) Ta[r] = 0.0;
+#pragma unroll kRtUnroll
+        for (int n = 1; n < ncut_rt; ++n) {
+            const double c = k.c2nL[n], b = k.n2L2[n], d = k.dn[n];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double B  = q[r] + b;
+                const double wp = inv_cube_sqrt_far<O2>(fma(-c, arz[r], B));
+                const double wm = inv_cube_sqrt_far<O2>(fma(c, arz[r], B));
+                S[r] = __dadd_rn(S[r], wp);          // not contracted with w = c g: that DFMA would have three register sources
+                S[r] = __dadd_rn(S[r], wm);
+                Ta[r] = fma(d, wp - wm, Ta[r]);
+            }
+        }
+        const double ce = k.c2nL[ncut_rt], be = k.n2L2[ncut_rt], de = k.dn[ncut_rt];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double we = inv_cube_sqrt_far<O2>(fma(-ce, arz[r], q[r] + be));
+            we = ((hi32(arz[r]) & 0x7fffffff) | lo32(arz[r])) != 0 ? we : 0.0;
+            S[r] = __dadd_rn(S[r], we);
+            Ta[r] = fma(de, we, Ta[r]);
+        }
+    } else {
+        // N_cut beyond the tabulated constants: they are formed in the loop
+#pragma unroll
+        for (int r = 0; r < R; ++r) Ta[r] = 0.0;
+        for (int n = 1; n < ncut_rt; ++n) {
+            const double nL = (double)n * k.L, t = 2.0 * nL;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double B  = fma(nL, nL, q[r]);
+                const double wp = inv_cube_sqrt(fma(-t, arz[r], B));
+                const double wm = inv_cube_sqrt(fma(t, arz[r], B));
+                S[r] = __dadd_rn(S[r], wp);          // not contracted with w = c g: that DFMA would have three register sources
+                S[r] = __dadd_rn(S[r], wm);
+                Ta[r] = fma((double)n, wp - wm, Ta[r]);
+            }
+        }
+        const double NL = (double)ncut_rt * k.L;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double we = inv_cube_sqrt(fma(-2.0 * NL, arz[r], fma(NL, NL, q[r])));
+            we = ((hi32(arz[r]) & 0x7fffffff) | lo32(arz[r])) != 0 ? we : 0.0;
+            S[r] = __dadd_rn(S[r], we);
+            Ta[r] = fma((double)ncut_rt, we, Ta[r]);
+        }
     }
 }
 

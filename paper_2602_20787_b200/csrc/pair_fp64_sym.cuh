@@ -49,17 +49,20 @@ constexpr int kSymUnroll = STEPS_SYM_UNROLL;
 struct __align__(16) SymSrc { double x, y, z, m, h, pad; };
 
 // Targets a lane keeps in registers (R = SYM_R of them, one per target tile of the CTA).
-struct SymTgt { double x, y, z, h, m, mL; };         // mL = -L m
+struct SymTgt { double x, y, z, h, m; };
 
 // 32 ring steps of one warp against one 32-source sub-tile.  R targets per lane meet the same
 // source in a step, so the source record is loaded and its accumulators are shuffled once per R
-// pairs.  SYM: also accumulate on the sources.  Source-side accumulators (rotating):
-// bx = sum m_i S r_x, by = sum m_i S r_y, bz = sum m_i (S r_z - L T) -- z already combined,
-// so only three values travel.
+// pairs.  SYM: also accumulate on the sources.  Per pair, with (S, T) the image sums,
+//     P = (S r_x, S r_y, S r_z - L T)          -- the pair's acceleration per unit G m, sign included
+//     target i:  a   += m_j P        source j (rotating accumulators):  b += m_i P   (subtracted at the flush)
+// so the three products P are formed once and serve both particles, and only three values travel.
+// (FP64 instructions with three distinct register sources -- the six multiply-adds above -- take three issue
+// cycles, all others two: profiles/r2_fp64_pipe_microbench.md.)
 template <int NC, int R, bool SYM, bool O2, bool GENERAL = false, class KC = PairConsts>
 __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&soft_hi)[R],
                                              const SymSrc *s_src, int lane, const KC &k,
-                                             int ncut_rt, double (&a)[R][4], double &bx,
+                                             int ncut_rt, double (&a)[R][3], double &bx,
                                              double &by, double &bz)
 {
     bx = by = bz = 0.0;
@@ -69,75 +72,48 @@ __device__ __forceinline__ void ring_subtile(const SymTgt (&ti)[R], const int (&
         const double2 pa = *reinterpret_cast<const double2 *>(&sj->x);
         const double2 pb = *reinterpret_cast<const double2 *>(&sj->z);
         const double hj = sj->h;
+        double rx[R], ry[R], rz[R], U[R], S[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            rx[r] = ti[r].x - pa.x;
+            ry[r] = ti[r].y - pa.y;
+            rz[r] = nearest_image(ti[r].z - pb.x, k);
+        }
         if constexpr (GENERAL) {
             // general path (2 max h > L/2): the literal image loop of Eq. 8 with every image through the spline
             // test; (S, T) serve both particles of the pair exactly as on the fast path
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
-                const double rz = nearest_image(ti[r].z - pb.x, k);
-                double S, T;
-                image_sum_general(rz, fma(ry, ry, rx * rx), ti[r].h + hj, k, ncut_rt, S, T);
-                const double Sj = pb.y * S;
-                a[r][0] = fma(Sj, rx, a[r][0]);
-                a[r][1] = fma(Sj, ry, a[r][1]);
-                a[r][2] = fma(Sj, rz, a[r][2]);
-                a[r][3] = fma(pb.y, T, a[r][3]);
-                if (SYM) {
-                    const double Si = ti[r].m * S;
-                    bx = fma(Si, rx, bx);
-                    by = fma(Si, ry, by);
-                    bz = fma(Si, rz, bz);
-                    bz = fma(ti[r].mL, T, bz);
-                }
+                double T;
+                image_sum_general(rz[r], fma(ry[r], ry[r], rx[r] * rx[r]), ti[r].h + hj, k, ncut_rt, S[r], T);
+                U[r] = fma(-k.L, T, S[r] * rz[r]);
             }
-        } else if constexpr (NC == 0) {
-            // run-time N_cut: all R targets go through the image loop together (image_sum_rt)
-            double rx[R], ry[R], rz[R], q[R], hi[R], S[R], T[R];
+        } else {
+            double arz[R], q[R], hi[R], Ta[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                rx[r] = ti[r].x - pa.x;
-                ry[r] = ti[r].y - pa.y;
-                rz[r] = nearest_image(ti[r].z - pb.x, k);
+                arz[r] = fabs(rz[r]);
                 q[r] = fma(rz[r], rz[r], fma(ry[r], ry[r], rx[r] * rx[r]));
                 hi[r] = ti[r].h;
             }
-            image_sum_rt<R, O2>(rz, q, hi, hj, soft_hi, k, ncut_rt, S, T);
+            image_sums<NC, R, O2>(arz, q, hi, hj, soft_hi, k, ncut_rt, S, Ta);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const double Sj = pb.y * S[r];
-                a[r][0] = fma(Sj, rx[r], a[r][0]);
-                a[r][1] = fma(Sj, ry[r], a[r][1]);
-                a[r][2] = fma(Sj, rz[r], a[r][2]);
-                a[r][3] = fma(pb.y, T[r], a[r][3]);
-                if (SYM) {
-                    const double Si = ti[r].m * S[r];
-                    bx = fma(Si, rx[r], bx);
-                    by = fma(Si, ry[r], by);
-                    bz = fma(Si, rz[r], bz);
-                    bz = fma(ti[r].mL, T[r], bz);
-                }
+                // sign(r_z) (S |r_z| - L Ta): the sign goes back on with one integer op on the high word
+                const double Ua = fma(-k.L, Ta[r], S[r] * arz[r]);
+                U[r] = __hiloint2double(hi32(Ua) ^ (hi32(rz[r]) & 0x80000000), lo32(Ua));
             }
-        } else
+        }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const double rx = ti[r].x - pa.x, ry = ti[r].y - pa.y;
-            const double rz = nearest_image(ti[r].z - pb.x, k);
-            const double rho2 = fma(ry, ry, rx * rx);
-            const double q = fma(rz, rz, rho2);
-            double S, T;
-            image_sum<NC, O2>(rz, q, ti[r].h, hj, soft_hi[r], k, ncut_rt, S, T);
-            const double Sj = pb.y * S;
-            a[r][0] = fma(Sj, rx, a[r][0]);
-            a[r][1] = fma(Sj, ry, a[r][1]);
-            a[r][2] = fma(Sj, rz, a[r][2]);
-            a[r][3] = fma(pb.y, T, a[r][3]);
+            const double Px = S[r] * rx[r], Py = S[r] * ry[r];
+            a[r][0] = fma(pb.y, Px, a[r][0]);
+            a[r][1] = fma(pb.y, Py, a[r][1]);
+            a[r][2] = fma(pb.y, U[r], a[r][2]);
             if (SYM) {
-                const double Si = ti[r].m * S;
-                bx = fma(Si, rx, bx);
-                by = fma(Si, ry, by);
-                bz = fma(Si, rz, bz);
-                bz = fma(ti[r].mL, T, bz);
+                bx = fma(ti[r].m, Px, bx);
+                by = fma(ti[r].m, Py, by);
+                bz = fma(ti[r].m, U[r], bz);
             }
         }
         if (SYM) {
@@ -161,7 +137,7 @@ struct SymSmem {
 };
 
 // acc layout: acc[comp * n_pad + particle], comp = 0..3 (A_x, A_y, A_z1, A_z2), zeroed by prestep_kernel
-// before the launch; the source side adds its combined z sum to A_z1.
+// before the launch; these kernels add the combined z sum S r_z - L T to A_z1 and leave A_z2 zero.
 // grid = (n_tiles / SYM_R, chunks).  CTA (bi, c): target tiles SYM_R*bi + r (lane holds particle
 // tid of each), source tiles [c*tpc, (c+1)*tpc) from SYM_R*bi on.
 // GENERAL: the same decomposition with the general pair law (ring_subtile<..., GENERAL>).
@@ -184,14 +160,13 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
     const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA takes
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     SymTgt ti[SYM_R];
-    double a[SYM_R][4];
+    double a[SYM_R][3];
 #pragma unroll
     for (int r = 0; r < SYM_R; ++r) {
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
         const double2 pi = xy[i], qi = zm[i];
         ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
-        ti[r].mL = -k.L * qi.y;
-        a[r][0] = a[r][1] = a[r][2] = a[r][3] = 0.0;
+        a[r][0] = a[r][1] = a[r][2] = 0.0;
     }
 
     for (int t = t0; t < t1; ++t) {
@@ -229,7 +204,7 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
                     if (tb + r > t) continue;
                     const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
                     const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
-                    double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
+                    double (&a1r)[1][3] = reinterpret_cast<double (&)[1][3]>(a[r]);
                     double cx = 0.0, cy = 0.0, cz = 0.0;
                     if (tb + r < t || js > w)
                         ring_subtile<NC, 1, true, O2, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
@@ -256,7 +231,7 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
     for (int r = 0; r < SYM_R; ++r) {
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
+        for (int c = 0; c < 3; ++c) atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
     }
 }
 
@@ -325,7 +300,7 @@ __device__ __forceinline__ void round_body(const double2 *__restrict__ xy, const
     if (SPLIT) acc_i += (size_t)blockIdx.y * 4 * n_pad;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     SymTgt ti[SYM_R];
-    double a[SYM_R][4];
+    double a[SYM_R][3];
     int soft_hi[SYM_R];
     const double hm = tile_hmax[t];
 #pragma unroll
@@ -333,8 +308,7 @@ __device__ __forceinline__ void round_body(const double2 *__restrict__ xy, const
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
         const double2 pi = xy[i], qi = zm[i];
         ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
-        ti[r].mL = -k.L * qi.y;
-        a[r][0] = a[r][1] = a[r][2] = a[r][3] = 0.0;
+        a[r][0] = a[r][1] = a[r][2] = 0.0;
         const double b = ti[r].h + hm;
         soft_hi[r] = hi32(b * b);
     }
@@ -358,7 +332,7 @@ __device__ __forceinline__ void round_body(const double2 *__restrict__ xy, const
                 if (mode[r] == 0) continue;
                 const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
                 const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
-                double (&a1r)[1][4] = reinterpret_cast<double (&)[1][4]>(a[r]);
+                double (&a1r)[1][3] = reinterpret_cast<double (&)[1][3]>(a[r]);
                 double cx = 0.0, cy = 0.0, cz = 0.0;
                 if (mode[r] == 1 || js > w)
                     ring_subtile<NC, 1, true, false, GENERAL, KC>(t1r, s1r, sub, lane, k, ncut_rt, a1r, cx, cy, cz);
@@ -387,7 +361,7 @@ __device__ __forceinline__ void round_body(const double2 *__restrict__ xy, const
         if (mode[r] == 0) continue;
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < 3; ++c) {
             double *p = acc_i + (size_t)c * n_pad + i;        // only the owner CTA ever writes these
             *p = *p + a[r][c];
         }

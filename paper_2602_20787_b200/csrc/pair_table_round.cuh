@@ -67,7 +67,6 @@ pair_table_round_kernel(const double2 *__restrict__ xy, const double2 *__restric
             const int i = (tb + r) * PAIR_THREADS + tq;
             const double2 pi = xy[i], qi = zm[i];
             ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
-            ti[r].mL = 0.0;
             a[r][0] = a[r][1] = a[r][2] = 0.0;
             const double bb = ti[r].h + hm;
             soft_hi[r] = hi32(bb * bb);

@@ -328,7 +328,6 @@ pair_table_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict_
         const int i = (tgt0 + r) * PAIR_THREADS + wq * 32 + lane;
         const double2 pi = xy[i], qi = zm[i];
         ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
-        ti[r].mL = 0.0;
         a[r][0] = a[r][1] = a[r][2] = 0.0;
     }
     for (int t = t0; t < t1; ++t) {
