@@ -112,29 +112,32 @@ prestep_kernel(double *__restrict__ x, double *__restrict__ y, double *__restric
                double2 *__restrict__ xy, double2 *__restrict__ zm, double *__restrict__ hs,
                float4 *__restrict__ f_hi, float4 *__restrict__ f_lo, double *__restrict__ tile_hmax,
                DevFlags *__restrict__ flags, int *__restrict__ bad_h_sticky,
-               double *__restrict__ part, int zero_rows)
+               double *__restrict__ part, int zero_rows, const int *__restrict__ perm)
 {
     const int lane = threadIdx.x & 31;
     const int i = (LANES == 32) ? blockIdx.x * OnStep<LANES>::kParticlesPerBlock + (threadIdx.x >> 5)
                                 : blockIdx.x * PAIR_THREADS + threadIdx.x;           // < n_pad
+    // i: slot in the packed arrays; p: the caller's index of the particle that sits there (perm: the spatial
+    // ordering of the EWALD_TABLE kernels, order_kernels.cuh; nullptr = caller order)
+    const int p = (perm != nullptr && i < n) ? perm[i] : i;
     double xv, yv, zv, mv, hv;
     if (i < n) {
-        xv = x[i]; yv = y[i];
+        xv = x[p]; yv = y[p];
         double sb = 0.0;
         if (KICK) sb = background_scale<LANES>(xv, yv, bg, lane);
         if (LANES == 32 && lane != 0) return;
-        zv = z[i]; mv = m[i]; hv = h[i];
+        zv = z[p]; mv = m[p]; hv = h[p];
         if (KICK) {
             const double hdt = 0.5 * kp.dt;
-            double ux = vx[i], uy = vy[i], uz = vz[i];
-            ux = ux + hdt * ((gx[i] + sb * xv) * kp.inv_a3 - 2.0 * kp.H * ux);
-            uy = uy + hdt * ((gy[i] + sb * yv) * kp.inv_a3 - 2.0 * kp.H * uy);
-            uz = uz + hdt * (gz[i] * kp.inv_a3 - 2.0 * kp.H * uz);
-            vx[i] = ux; vy[i] = uy; vz[i] = uz;
+            double ux = vx[p], uy = vy[p], uz = vz[p];
+            ux = ux + hdt * ((gx[p] + sb * xv) * kp.inv_a3 - 2.0 * kp.H * ux);
+            uy = uy + hdt * ((gy[p] + sb * yv) * kp.inv_a3 - 2.0 * kp.H * uy);
+            uz = uz + hdt * (gz[p] * kp.inv_a3 - 2.0 * kp.H * uz);
+            vx[p] = ux; vy[p] = uy; vz[p] = uz;
             xv = xv + ux * kp.dt;
             yv = yv + uy * kp.dt;
             zv = wrap_z(zv + uz * kp.dt, L);
-            x[i] = xv; y[i] = yv; z[i] = zv;
+            x[p] = xv; y[p] = yv; z[p] = zv;
         } else {
             zv = wrap_z(zv, L);
         }
@@ -189,7 +192,7 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
                 double *__restrict__ gx, double *__restrict__ gy, double *__restrict__ gz,
                 const double *__restrict__ x, const double *__restrict__ y,
                 double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
-                BgParams bg, KickParams kp)
+                BgParams bg, KickParams kp, const int *__restrict__ perm)
 {
     const int lane = threadIdx.x & 31;
     const int i = (LANES == 32) ? blockIdx.x * OnStep<LANES>::kParticlesPerBlock + (threadIdx.x >> 5)
@@ -197,9 +200,10 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
     if (blockIdx.x == 0 && threadIdx.x == 0) { flags_next->hmax_bits = 0ull; flags_next->bad_h = 0; }
     if ((i % PAIR_THREADS) == 0 && lane == 0) tile_hmax[i / PAIR_THREADS] = 0.0;
     if (i >= n) return;
+    const int p = (perm != nullptr) ? perm[i] : i;      // slot i of the packed arrays holds the caller's particle p
     double sb = 0.0, xv = 0.0, yv = 0.0;
     if (KICK) {
-        xv = x[i]; yv = y[i];
+        xv = x[p]; yv = y[p];
         sb = background_scale<LANES>(xv, yv, bg, lane);
     }
     if (LANES == 32 && lane != 0) return;
@@ -212,12 +216,12 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
         a3 += p[3 * (size_t)n_pad];
     }
     const double g0 = -G * a0, g1 = -G * a1, g2 = -G * fma(-L, a3, a2);
-    gx[i] = g0; gy[i] = g1; gz[i] = g2;
+    gx[p] = g0; gy[p] = g1; gz[p] = g2;
     if (KICK) {
         const double hdt = 0.5 * kp.dt, den = 1.0 + kp.H * kp.dt;
-        vx[i] = (vx[i] + hdt * (g0 + sb * xv) * kp.inv_a3) / den;
-        vy[i] = (vy[i] + hdt * (g1 + sb * yv) * kp.inv_a3) / den;
-        vz[i] = (vz[i] + hdt * g2 * kp.inv_a3) / den;
+        vx[p] = (vx[p] + hdt * (g0 + sb * xv) * kp.inv_a3) / den;
+        vy[p] = (vy[p] + hdt * (g1 + sb * yv) * kp.inv_a3) / den;
+        vz[p] = (vz[p] + hdt * g2 * kp.inv_a3) / den;
     }
 }
 

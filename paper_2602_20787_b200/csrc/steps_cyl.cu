@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "aux_kernels.cuh"
+#include "order_kernels.cuh"
 #include "pair_fp64.cuh"
 #include "pair_fp64_sym.cuh"
 #include "pair_mixed.cuh"
@@ -53,6 +54,11 @@ struct steps_cyl_ctx {
     DevFlags *cur_flags = nullptr;                 // the block of the evaluation being enqueued
     int *bad_h_sticky = nullptr;                   // h <= 0 seen since the last steps_cyl_check
     unsigned eval_count = 0;
+    // spatial ordering of the packed arrays (EWALD_TABLE mode, order_kernels.cuh)
+    bool use_order = false;
+    int n_pow2 = 0;
+    int *perm = nullptr;                           // packed slot -> caller index
+    unsigned long long *order_keys = nullptr, *rmax_bits = nullptr;
     GraphSlot gslot[2];                            // STEPS_FLAG_GRAPH: one captured evaluation per flag-block parity
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
@@ -423,11 +429,12 @@ struct PreVals {
     int *sticky;
     double *part;
     int zero_rows;
-    void *args[26];
+    const int *perm;
+    void *args[27];
     void bind()
     {
-        void *a[26] = {&x, &y, &z, &vx, &vy, &vz, &gx, &gy, &gz, &m, &h, &n, &n_pad, &L, &bg, &kp, &xy, &zm, &hs,
-                       &f_hi, &f_lo, &tile_hmax, &fl, &sticky, &part, &zero_rows};
+        void *a[27] = {&x, &y, &z, &vx, &vy, &vz, &gx, &gy, &gz, &m, &h, &n, &n_pad, &L, &bg, &kp, &xy, &zm, &hs,
+                       &f_hi, &f_lo, &tile_hmax, &fl, &sticky, &part, &zero_rows, &perm};
         std::memcpy(args, a, sizeof a);
     }
 };
@@ -442,11 +449,12 @@ struct PostVals {
     double *vx, *vy, *vz;
     BgParams bg;
     KickParams kp;
-    void *args[18];
+    const int *perm;
+    void *args[19];
     void bind()
     {
-        void *a[18] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &tile_hmax, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz,
-                       &bg, &kp};
+        void *a[19] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &tile_hmax, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz,
+                       &bg, &kp, &perm};
         std::memcpy(args, a, sizeof a);
     }
 };
@@ -505,6 +513,7 @@ void fill_vals(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, PreVals 
     post.vx = pre.vx; post.vy = pre.vy; post.vz = pre.vz;
     post.bg = pre.bg;
     post.kp = kick ? kick->k2 : none;
+    pre.perm = post.perm = ctx->use_order ? ctx->perm : nullptr;
 }
 
 int enqueue_force_plain(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, bool timed, cudaStream_t s)
@@ -600,11 +609,44 @@ int enqueue_force_graph(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity,
     return STEPS_OK;
 }
 
+// perm <- the particles' order along a Morton curve through their current positions (order_kernels.cuh): key
+// generation, a bitonic sort of the (key, index) words -- chunks of 1024 in shared memory, larger strides one pass
+// per launch -- and the extraction of the indices.  O(N log^2 N), a few ms at N = 4 M, once per kReorderEvery calls.
+int enqueue_reorder(steps_cyl_ctx *ctx, const double *x, const double *y, const double *z, cudaStream_t s)
+{
+    constexpr int T = 512, CHUNK = 2 * T;
+    const int tb = 256, np2 = ctx->n_pow2;
+    CK(cudaMemsetAsync(ctx->rmax_bits, 0, sizeof(unsigned long long), s));
+    extent_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(x, y, ctx->n, ctx->rmax_bits);
+    order_key_kernel<<<(np2 + tb - 1) / tb, tb, 0, s>>>(x, y, z, ctx->n, np2, ctx->p.Lz, ctx->rmax_bits,
+                                                       ctx->order_keys);
+    bitonic_chunk_kernel<T><<<np2 / CHUNK, T, 0, s>>>(ctx->order_keys, 2, CHUNK);
+    ctx->launches += 3;
+    for (long long k = 2LL * CHUNK; k <= np2; k <<= 1) {
+        for (long long j = k >> 1; j >= CHUNK; j >>= 1) {
+            bitonic_pass_kernel<<<(np2 / 2 + tb - 1) / tb, tb, 0, s>>>(ctx->order_keys, np2, (int)j, (int)k);
+            ctx->launches += 1;
+        }
+        bitonic_chunk_kernel<T><<<np2 / CHUNK, T, 0, s>>>(ctx->order_keys, (int)k, (int)k);
+        ctx->launches += 1;
+    }
+    order_perm_kernel<<<(ctx->n + tb - 1) / tb, tb, 0, s>>>(ctx->order_keys, ctx->n, ctx->perm);
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return STEPS_OK;
+}
+
 int enqueue_force(steps_cyl_ctx *ctx, double *x, double *y, double *z, const double *m, const double *h,
                   double *gx, double *gy, double *gz, const KdkArgs *kick, cudaStream_t s)
 {
     const ForceArgs f = {x, y, z, m, h, gx, gy, gz, kick};
     const unsigned parity = ctx->eval_count & 1u;      // which of the two flag blocks this evaluation uses
+    // the ordering is a locality hint: refreshed now and then (inside a replayed graph: taken once, before capture)
+    if (ctx->use_order && (ctx->eval_count == 0 ||
+                           (!(ctx->p.flags & STEPS_FLAG_GRAPH) && ctx->eval_count % kReorderEvery == 0))) {
+        int rc = enqueue_reorder(ctx, x, y, z, s);
+        if (rc != STEPS_OK) return rc;
+    }
     ctx->eval_count += 1;
     if (ctx->p.flags & STEPS_FLAG_GRAPH) return enqueue_force_graph(ctx, f, parity, s);
     return enqueue_force_plain(ctx, f, parity, true, s);
@@ -782,6 +824,14 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         ctx->tc.inv_drho = (double)(pp.tab_nrho - 1) / pp.tab_rho_max;
         ctx->tc.inv_dz = (double)(pp.tab_nz - 1) / (0.5 * pp.Lz);
         ctx->tc.two_over_L = 2.0 / pp.Lz;
+        // spatially ordered packed arrays: the gathers of a warp then fall in one patch of the table
+        ctx->use_order = true;
+        ctx->n_pow2 = 1024;
+        while (ctx->n_pow2 < ctx->n) ctx->n_pow2 <<= 1;
+        A(dev_alloc(&ctx->perm, (size_t)ctx->n));
+        A(dev_alloc(&ctx->order_keys, (size_t)ctx->n_pow2));
+        A(dev_alloc(&ctx->rmax_bits, 1));
+        if (rc != STEPS_OK) return fail(rc);
     }
     A(cudaMemset(ctx->flags, 0, 3 * sizeof(DevFlags)));
     if (rc != STEPS_OK) return fail(rc);
@@ -800,7 +850,7 @@ void steps_cyl_destroy(steps_cyl_ctx *c)
         if (g.graph) cudaGraphDestroy(g.graph);
     }
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
+    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->perm); cudaFree(c->order_keys); cudaFree(c->rmax_bits); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);

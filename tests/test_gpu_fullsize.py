@@ -157,3 +157,13 @@ def test_config3_full_size_deterministic(torch_cuda, oracle, cfg_case):
     """STEPS_FLAG_DETERMINISTIC at the bench size (4098 round launches per evaluation at N = 1 048 576)."""
     w, idx, ref0 = cfg_case(3, 192, oracle)
     _check(_accel(torch_cuda, w, 0, 1), ref0, idx, w, 0, "cfg3 fp64_deterministic")
+
+
+def test_config3_full_size_far_order2(torch_cuda, oracle, cfg_case):
+    """STEPS_FLAG_FAR_ORDER2 at the bench size (the evidence DESIGN section 5.1 cites for keeping it opt-in): the
+    far images' rsqrt refinement stops after its linear term, so the error is two orders above the default's
+    round-off level, still far inside the 1e-10 bar."""
+    w, idx, ref0 = cfg_case(3, 192, oracle)
+    got = _accel(torch_cuda, w, 0, 2)
+    _check(got, ref0, idx, w, 0, "cfg3 fp64 far_order2")
+    assert _rel(got[idx], ref0).max() <= 1e-11

@@ -163,49 +163,75 @@ def test_stereographic_load_parity_and_near_equilibrium(torch_cuda, oracle):
     assert abs(np.mean(nr)) < 0.03 * abs(np.mean(gr))
 
 
-def test_glass_making_with_repulsive_gravity(torch_cuda):
-    """a comoving run with REPULSIVE gravity (G < 0; the Eq. 9 term flips sign with it) and
-    Hubble drag relaxes the particle load towards a glass: the residual |g + b| / |g| of the stereographic
-    load falls (0.15 -> ~0.05 within 60 steps at this size) while the drag removes the kinetic energy.
-    The paper runs this for 1e5-1e6 expansion factors; here only the onset is checked."""
+def test_glass_making_converges(torch_cuda, oracle):
+    """"comoving run with repulsive gravity + Hubble drag" turns the particle load into a glass.
+    The stereographic load (Eq. 21-22, N ~ 40 000) is integrated with G < 0 (the Eq. 9 term flips sign with it) in an
+    Einstein-de Sitter background whose density is the load's (H^2 = 8 pi |G| rho0 / (3 a^3)), logarithmic time steps
+    dt = 0.03 t, for 800 KDK steps = an expansion factor of 7e6 (the paper quotes 1e5-1e6).  Linear theory: with
+    repulsive gravity density perturbations oscillate with amplitude ~ a^(-1/4), so the residual force
+    |g + b| / |g| of the load (0.064 median) must fall by more than an order of magnitude while the drag removes
+    the kinetic energy.  The curve is printed (-s) and kept in profiles/r2_glass.md.  On the glass the pair sum is
+    then parity-checked against the oracle and is cancelled by the Eq. 9 term to < 0.5 %."""
     import math
     from paper_2602_20787_b200 import binding as b
     from paper_2602_20787_b200 import workloads
     torch = torch_cuda
-    w = workloads.stereographic_load(n_target=6000)
-    n, G = w.n, -1.0
+    w = workloads.stereographic_load(n_target=40000)
+    n, G, eta, n_steps = w.n, -1.0, 0.03, 800
     ctx = b.StepsCyl(n=n, Lz=w.Lz, G=G, n_cut=5, R_sim=w.R_sim, rho0=w.rho0)
     dev = {k: _dev(torch, getattr(w, k)) for k in ("x", "y", "z", "m", "h")}
     v = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(3)]
     g = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
     bx, by = torch.empty_like(g[0]), torch.empty_like(g[0])
     rho = np.hypot(w.x, w.y)
-    inner = torch.from_numpy((rho > 20.0) & (rho < 400.0)).cuda()
+    inner = torch.from_numpy((rho > 20.0) & (rho < 0.8 * w.R_sim)).cuda()
 
     def residual():
         ctx.background(dev["x"], dev["y"], bx, by)
         net = torch.sqrt((g[0] + bx) ** 2 + (g[1] + by) ** 2 + g[2] ** 2)[inner]
         tot = torch.sqrt(g[0] ** 2 + g[1] ** 2 + g[2] ** 2)[inner]
-        return float(torch.median(net / tot))
+        return float(torch.median(net / tot)), float(torch.quantile(net / tot, 0.9))
 
     ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
     r0 = residual()
-    t, a = 1.0, 1.0                                   # Einstein-de Sitter clock: a ~ t^(2/3), H = 2/(3t)
-    dt = 0.05 / math.sqrt(abs(G) * w.rho0)
-    speeds = []
-    for s in range(1, 61):
+    H0 = math.sqrt(8.0 * math.pi * abs(G) * w.rho0 / 3.0)
+    t0 = 2.0 / (3.0 * H0)
+    t, a = t0, 1.0
+    print("\n[glass] N=%d  step 0  a=1  residual median %.4f  p90 %.4f" % (n, r0[0], r0[1]))
+    curve, ke = [], []
+    for s in range(1, n_steps + 1):
+        dt = eta * t
         t1 = t + dt
-        a1 = a * (t1 / t) ** (2.0 / 3.0)
+        a1 = (t1 / t0) ** (2.0 / 3.0)
         ctx.kdk_step(dev["x"], dev["y"], dev["z"], *v, dev["m"], dev["h"], *g, a, 2.0 / (3.0 * t), a1,
                      2.0 / (3.0 * t1), dt)
         t, a = t1, a1
-        if s in (20, 60):
-            speeds.append(float(torch.sqrt(v[0] ** 2 + v[1] ** 2 + v[2] ** 2).mean()))
+        if s % 40 == 0:
+            r = residual()
+            e = float((dev["m"] * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2)).sum())
+            curve.append(r[0])
+            ke.append(e)
+            print("[glass] step %4d  a=%.3e  residual median %.4f  p90 %.4f  sum m v^2 = %.3e" % (s, a, r[0], r[1], e))
     ctx.check()
-    r1 = residual()
+    assert 0.04 < r0[0] < 0.10
+    assert curve[-1] < 0.02 and curve[-1] < r0[0] / 20.0, curve[-1]
+    assert abs(curve[-1] - curve[-3]) < 0.3 * curve[-1]            # a plateau, not a transient
+    assert all(math.isfinite(e) for e in ke) and ke[-1] < 1e-3 * ke[0]
+    # the glass: pair-sum parity on sampled targets, and equilibrium with the homogeneous-cylinder term
+    xg, yg, zg = (dev[k].cpu().numpy() for k in ("x", "y", "z"))
+    gg = np.stack([t_.cpu().numpy() for t_ in g], 1)
+    idx = workloads.sample_targets(n, 300, seed=7)
+    ref = np.stack(oracle.accel(xg, yg, zg, w.m, w.h, w.Lz, G, 5, targets=idx), 1)
+    e = np.linalg.norm(gg[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert e.max() <= 1e-10
+    ctx.background(dev["x"], dev["y"], bx, by)
+    net = gg.copy()
+    net[:, 0] += bx.cpu().numpy()
+    net[:, 1] += by.cpu().numpy()
+    sel = inner.cpu().numpy()
+    ratio = np.linalg.norm(net[sel], axis=1) / np.linalg.norm(gg[sel], axis=1)
+    assert np.median(ratio) < 0.005
     ctx.close()
-    assert 0.10 < r0 < 0.25 and r1 < 0.75 * r0, (r0, r1)
-    assert all(math.isfinite(sp) for sp in speeds) and speeds[1] < speeds[0]
 
 
 def test_step_is_three_launches_and_graph_replay_matches(torch_cuda, oracle):

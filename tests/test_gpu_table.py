@@ -305,3 +305,32 @@ def test_two_live_contexts_with_different_table_sizes(torch_cuda, oracle):
         assert e.max() <= FP32_TABLE_MAX and np.median(e) <= FP32_TABLE_MEDIAN
     for ctx in ctxs:
         ctx.close()
+
+
+@pytest.mark.parametrize("flags", [0, 8], ids=["plain", "graph"])
+def test_table_mode_kdk_across_a_reordering(torch_cuda, oracle, flags):
+    """EWALD_TABLE mode keeps its packed arrays in Morton order (order_kernels.cuh) and refreshes the order every 64
+    force evaluations; inputs and outputs stay in the CALLER's order.  70 KDK steps cross a re-ordering: the final
+    g must be the oracle's table-mode pair sum at the final positions, and m, h must come back untouched."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(1, n=3001, seed=41)
+    nrho, nz, rmax = 72, 64, 300.0
+    ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, periodic_mode=b.PERIODIC_EWALD_TABLE, tab_nrho=nrho, tab_nz=nz,
+                     tab_rho_max=rmax, flags=flags)
+    dev = {k: torch.from_numpy(np.ascontiguousarray(getattr(w, k))).cuda() for k in ("x", "y", "z", "m", "h")}
+    rng = np.random.default_rng(5)
+    v = [torch.from_numpy(rng.normal(0, 0.05, w.n)).cuda() for _ in range(3)]
+    g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+    for _ in range(70):
+        ctx.kdk_step(dev["x"], dev["y"], dev["z"], *v, dev["m"], dev["h"], *g, 1.0, 0.0, 1.0, 0.0, 0.02)
+    ctx.check()
+    x, y, z = (dev[k].cpu().numpy() for k in ("x", "y", "z"))
+    assert np.array_equal(dev["m"].cpu().numpy(), w.m) and np.array_equal(dev["h"].cpu().numpy(), w.h)
+    assert np.abs(x - w.x).max() > 0.01 and z.min() >= 0.0 and z.max() < w.Lz
+    D = oracle.ewald_table(w.Lz, 2.0 / w.Lz, 5, 12, nrho, nz, rmax)
+    ref = oracle.accel_table(x, y, z, w.m, w.h, w.Lz, w.G, D, rmax, 0)
+    assert rel_err([t.cpu().numpy() for t in g], ref).max() <= 1e-10
+    ctx.close()
