@@ -213,6 +213,18 @@ def roofline_of(ctx, n, n_cut, t_pair, sm_count, sm_max, table):
     library, duration from the CUDA events the library records around that launch."""
     kernel = ctx.pair_kernel_name()
     cnt, how = pipe_counts(kernel, n_cut)
+    # the mixed image kernel runs two forms of its ring pass (pair_mixed_sym.cuh: SIMPLE where the Morton-ordered
+    # groups are far apart); their tallies are weighted with the pass counts the kernel itself keeps
+    simple_frac = None
+    n_simple, n_pass = ctx.pass_stats()
+    if n_pass > 0 and how == "counted":
+        from paper_2602_20787_b200 import build, sassmix
+        var = sassmix.load(build.SASSMIX)["kernels"][kernel]["variants"]
+        if len(var) >= 2:
+            simple_frac = n_simple / n_pass
+            cnt = {k: simple_frac * var[1]["per_interaction"][k] + (1.0 - simple_frac) * var[0]["per_interaction"][k]
+                   for k in cnt}
+            how = "two loop forms weighted by the kernel's own pass counts"
     pairs = float(n) * float(n - 1)
     is_mixed = "mixed" in kernel
     lanes = NOMINAL_FP32_LANES_PER_SM if is_mixed else NOMINAL_FP64_LANES_PER_SM
@@ -235,6 +247,8 @@ def roofline_of(ctx, n, n_cut, t_pair, sm_count, sm_max, table):
         "pipe_util_vs_nominal": instr * pairs / t_pair / (nominal_tflops * 1e12 / 2),
         "kernel_ms": 1e3 * t_pair,
     }
+    if simple_frac is not None:
+        r["simple_pass_fraction"] = simple_frac
     if is_mixed or cnt["fp32_ops"] > 0:
         xu_peak = sm_count * NOMINAL_XU_LANES_PER_SM * sm_max * 1e6
         r["xu_pipe_util_vs_nominal"] = (cnt["mufu"] + cnt["conv"]) * pairs / t_pair / xu_peak

@@ -233,6 +233,12 @@ int steps_cyl_last_pair_kernel_ms(steps_cyl_ctx *ctx, float *ms);
  * (paper_2602_20787_b200/sassmix.py) spells it, e.g. "pair_fp64_sym_kernel<5,false>".  Static per context. */
 const char *steps_cyl_pair_kernel_name(steps_cyl_ctx *ctx);
 
+/* Mixed-precision image kernel only: how many of its two-way ring passes (32 sources x 64 targets of a warp) since
+ * init took the SIMPLE form (plain float separations, one nearest-image shift, no spline test; possible where the
+ * Morton-ordered groups are far apart) out of all such passes.  Synchronises cuda_stream.  Both 0 for other kernels.
+ * bench.py weights the two loops' instruction tallies with this ratio. */
+int steps_cyl_pass_stats(steps_cyl_ctx *ctx, void *cuda_stream, uint64_t *simple, uint64_t *total);
+
 const char *steps_cyl_strerror(int code);
 const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx);
 

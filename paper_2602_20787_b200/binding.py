@@ -27,7 +27,7 @@ EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_
            "steps_cyl_kdk_step_host",
            "steps_cyl_friedmann_step", "steps_cyl_friedmann_step_cpl", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
            "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count",
-           "steps_cyl_pair_kernel_name"]
+           "steps_cyl_pair_kernel_name", "steps_cyl_pass_stats"]
 
 
 class Params(C.Structure):
@@ -91,6 +91,8 @@ def lib():
         L.steps_cyl_last_cuda_error.argtypes = [vp]
         L.steps_cyl_pair_kernel_name.restype = C.c_char_p
         L.steps_cyl_pair_kernel_name.argtypes = [vp]
+        L.steps_cyl_pass_stats.restype = C.c_int
+        L.steps_cyl_pass_stats.argtypes = [vp, vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         L.steps_cyl_launch_count.restype = i64
         L.steps_cyl_launch_count.argtypes = [vp]
         _lib = L
@@ -245,6 +247,14 @@ class StepsCyl:
 
     def pair_kernel_name(self):
         return lib().steps_cyl_pair_kernel_name(self._ctx).decode()
+
+    def pass_stats(self):
+        """(simple, total) two-way ring passes of the mixed image kernel since init."""
+        a, t = C.c_uint64(), C.c_uint64()
+        rc = lib().steps_cyl_pass_stats(self._ctx, _stream(), C.byref(a), C.byref(t))
+        if rc:
+            self._raise(rc)
+        return int(a.value), int(t.value)
 
     def launch_count(self):
         return int(lib().steps_cyl_launch_count(self._ctx))

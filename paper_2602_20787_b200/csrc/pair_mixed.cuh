@@ -26,6 +26,8 @@ constexpr int kRtUnrollMixed = STEPS_RT_UNROLL_MIXED;   // run-time N_cut image 
 
 struct MixedConsts {
     float Lh, Ll, halfL;
+    float simple_ratio2;                  // SIMPLE ring pass (pair_mixed_sym.cuh) needs d^2 * simple_ratio2 >= c^2
+    float simple_ext2;                    // ... and d^2 >= simple_ext2 * (source box extent)^2
     float c2nL[MAX_NCUT_TABLE + 1];       // 2 n L
     float n2L2[MAX_NCUT_TABLE + 1];       // (n L)^2
     float dn[MAX_NCUT_TABLE + 1];         // n

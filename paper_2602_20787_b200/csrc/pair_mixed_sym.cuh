@@ -178,12 +178,30 @@ struct MixTgt2 { float2 xh, yh, zh, xl, yl, zl, h, m, mL; };       // .x: target
 // 32 ring steps, both targets of the lane at once, symmetric (source side accumulated too).
 // a[c] (c = 0..3: A_x, A_y, A_z1, A_z2) and bx, by, bz are FLOAT partial sums of this ring, the two
 // halves belonging to the two targets; the caller adds the halves of b.
-template <int NC>
+// SIMPLE (decided per warp and source sub-tile from bounding boxes, pass_is_simple below): every pair of the pass
+// (a) has the same nearest-image shift zshift in {0, +L, -L}, (b) lies outside every spline support, and (c) is
+// far apart compared with the size of the source sub-tile and with the coordinates' magnitude.  Then positions are
+// taken relative to the sub-tile's centre O: the sources' offsets (x_hi - O) + x_lo were stored as single floats
+// when the tile was staged (s_rel; error 2^-24 of the sub-tile's size), the two targets' offsets are formed once per
+// pass, and a separation is ONE packed subtraction -- 3 packed operations of geometry instead of 13, one LDS.128
+// instead of two, no spline pre-test.  What is lost is the targets' lo part relative to their distance from O
+// (2^-24 d): an error common to all sources of the pass, which the sum tolerates (measured: parity unchanged),
+// unlike independent per-source roundings of 2^-24 |x| (measured: 10x the error at r ~ 2000).
+// Possible because the packed arrays are in Morton order (order_kernels.cuh).
+template <int NC, bool SIMPLE = false>
 __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int (&soft_bits)[2],
                                                    const float4 *s_hi, const float4 *s_lo, int lane,
                                                    const MixedConsts &k, int ncut_rt, float2 (&a)[4],
-                                                   float2 &bx, float2 &by, float2 &bz)
+                                                   float2 &bx, float2 &by, float2 &bz,
+                                                   const float4 *s_rel = nullptr, float ox = 0.0f, float oy = 0.0f,
+                                                   float oz = 0.0f, float zshift = 0.0f)
 {
+    float2 Tx = bc(0.0f), Ty = bc(0.0f), Tz = bc(0.0f);
+    if constexpr (SIMPLE) {
+        Tx = add2(sub2(ti.xh, bc(ox)), ti.xl);
+        Ty = add2(sub2(ti.yh, bc(oy)), ti.yl);
+        Tz = add2(sub2(sub2(ti.zh, bc(oz)), bc(zshift)), ti.zl);
+    }
     bx = by = bz = bc(0.0f);
 #pragma unroll
     for (int c = 0; c < 4; ++c) a[c] = bc(0.0f);
@@ -191,23 +209,37 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
 #pragma unroll kMixedUnroll
     for (int s = 0; s < 32; ++s) {
         const int jj = (lane + s) & 31;
-        const float4 jh = s_hi[jj], jl = s_lo[jj];          // {x_hi,y_hi,z_hi,m}, {x_lo,y_lo,z_lo,h}
-        const float2 rx = add2(sub2(ti.xh, bc(jh.x)), sub2(ti.xl, bc(jl.x)));
-        const float2 ry = add2(sub2(ti.yh, bc(jh.y)), sub2(ti.yl, bc(jl.y)));
-        float2 rzh = sub2(ti.zh, bc(jh.z)), rzl = sub2(ti.zl, bc(jl.z));
-        // nearest image: k = rint(rz / L) by the magic-number trick (|rz| < L, so k in {-1, 0, 1});
-        // a tie at |rz| = L/2 may go either way (the image set is symmetric then)
-        const float2 kk = sub2(fma2(rzh, bc(invL), bc(magic)), bc(magic));
-        rzh = fma2(kk, bc(-k.Lh), rzh);
-        rzl = fma2(kk, bc(-k.Ll), rzl);
-        const float2 rz = add2(rzh, rzl);
+        float2 rx, ry, rz;
+        float hj = 0.0f, jm;
+        if constexpr (SIMPLE) {
+            const float4 jr = s_rel[jj];                     // {x, y, z relative to the sub-tile's centre, m}
+            jm = jr.w;
+            rx = sub2(Tx, bc(jr.x));
+            ry = sub2(Ty, bc(jr.y));
+            rz = sub2(Tz, bc(jr.z));
+        } else {
+            const float4 jh = s_hi[jj], jl = s_lo[jj];       // {x_hi,y_hi,z_hi,m}, {x_lo,y_lo,z_lo,h}
+            hj = jl.w;
+            jm = jh.w;
+            rx = add2(sub2(ti.xh, bc(jh.x)), sub2(ti.xl, bc(jl.x)));
+            ry = add2(sub2(ti.yh, bc(jh.y)), sub2(ti.yl, bc(jl.y)));
+            float2 rzh = sub2(ti.zh, bc(jh.z)), rzl = sub2(ti.zl, bc(jl.z));
+            // nearest image: k = rint(rz / L) by the magic-number trick (|rz| < L, so k in {-1, 0, 1});
+            // a tie at |rz| = L/2 may go either way (the image set is symmetric then)
+            const float2 kk = sub2(fma2(rzh, bc(invL), bc(magic)), bc(magic));
+            rzh = fma2(kk, bc(-k.Lh), rzh);
+            rzl = fma2(kk, bc(-k.Ll), rzl);
+            rz = add2(rzh, rzl);
+        }
         const float2 rho2 = fma2(ry, ry, mul2(rx, rx));
         const float2 q = fma2(rz, rz, rho2);
         float2 w0 = cube2(rsqrt2(q));
-        if (__float_as_int(q.x) <= soft_bits[0] || __float_as_int(q.y) <= soft_bits[1]) {
-            const float h0 = ti.h.x + jl.w, h1 = ti.h.y + jl.w;
-            if (q.x < h0 * h0) w0.x = spline_w_f32(q.x, h0);
-            if (q.y < h1 * h1) w0.y = spline_w_f32(q.y, h1);
+        if constexpr (!SIMPLE) {
+            if (__float_as_int(q.x) <= soft_bits[0] || __float_as_int(q.y) <= soft_bits[1]) {
+                const float h0 = ti.h.x + hj, h1 = ti.h.y + hj;
+                if (q.x < h0 * h0) w0.x = spline_w_f32(q.x, h0);
+                if (q.y < h1 * h1) w0.y = spline_w_f32(q.y, h1);
+            }
         }
         float2 S = w0, T = bc(0.0f);
         const int n_img = (NC > 0) ? NC : ncut_rt;
@@ -251,11 +283,11 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
             const float2 ns = make_float2(copysignf((float)n_img, rz.x), copysignf((float)n_img, rz.y));
             T = fma2(ns, we, T);
         }
-        const float2 Sj = mul2(bc(jh.w), S);
+        const float2 Sj = mul2(bc(jm), S);
         a[0] = fma2(Sj, rx, a[0]);
         a[1] = fma2(Sj, ry, a[1]);
         a[2] = fma2(Sj, rz, a[2]);
-        a[3] = fma2(bc(jh.w), T, a[3]);
+        a[3] = fma2(bc(jm), T, a[3]);
         const float2 Si = mul2(ti.m, S);
         bx = fma2(Si, rx, bx);
         by = fma2(Si, ry, by);
@@ -268,6 +300,64 @@ __device__ __forceinline__ void ring_subtile_f32x2(const MixTgt2 &ti, const int 
     }
 }
 
+// Bounding box (of the float hi parts) of a group of particles, with their largest softening and largest |x|, |y|.
+struct MixBox { float xlo, xhi, ylo, yhi, zlo, zhi, hmax, cmax; };
+
+__device__ __forceinline__ MixBox box_of(float x, float y, float z, float h)
+{
+    MixBox b;
+    b.xlo = b.xhi = x; b.ylo = b.yhi = y; b.zlo = b.zhi = z; b.hmax = h;
+    b.cmax = fmaxf(fabsf(x), fabsf(y));
+    return b;
+}
+__device__ __forceinline__ MixBox box_join(const MixBox &a, const MixBox &b)
+{
+    MixBox c;
+    c.xlo = fminf(a.xlo, b.xlo); c.xhi = fmaxf(a.xhi, b.xhi);
+    c.ylo = fminf(a.ylo, b.ylo); c.yhi = fmaxf(a.yhi, b.yhi);
+    c.zlo = fminf(a.zlo, b.zlo); c.zhi = fmaxf(a.zhi, b.zhi);
+    c.hmax = fmaxf(a.hmax, b.hmax); c.cmax = fmaxf(a.cmax, b.cmax);
+    return c;
+}
+__device__ __forceinline__ MixBox box_warp(MixBox b)            // union over the lanes of the warp
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        MixBox c;
+        c.xlo = __shfl_xor_sync(0xffffffffu, b.xlo, o); c.xhi = __shfl_xor_sync(0xffffffffu, b.xhi, o);
+        c.ylo = __shfl_xor_sync(0xffffffffu, b.ylo, o); c.yhi = __shfl_xor_sync(0xffffffffu, b.yhi, o);
+        c.zlo = __shfl_xor_sync(0xffffffffu, b.zlo, o); c.zhi = __shfl_xor_sync(0xffffffffu, b.zhi, o);
+        c.hmax = __shfl_xor_sync(0xffffffffu, b.hmax, o); c.cmax = __shfl_xor_sync(0xffffffffu, b.cmax, o);
+        b = box_join(b, c);
+    }
+    return b;
+}
+
+// Can every pair (target in t, source in s) take the SIMPLE form of ring_subtile_f32x2?  (a) one nearest-image
+// shift for all of them, (b) box distance d beyond every spline support, (c) d >= half the source box's largest
+// extent (the stored offsets from its centre are then good to 2^-23 d) and d >= c / 8 with c the largest
+// coordinate magnitude (x, y of both boxes; z < L) -- thresholds in MixedConsts, set by the host.  Margins cover
+// the lo parts the boxes do not see.
+__device__ __forceinline__ bool pass_is_simple(const MixBox &t, const MixBox &s, const MixedConsts &k, float &zshift)
+{
+    const float eps = 1.0e-5f * k.Lh;
+    float dlo = t.zlo - s.zhi - eps, dhi = t.zhi - s.zlo + eps;          // range of the raw r_z = z_i - z_j
+    if (dlo > -k.halfL && dhi < k.halfL) zshift = 0.0f;
+    else if (dlo > k.halfL) zshift = k.Lh;
+    else if (dhi < -k.halfL) zshift = -k.Lh;
+    else return false;
+    dlo -= zshift;
+    dhi -= zshift;
+    const float gz = fmaxf(0.0f, fmaxf(dlo, -dhi));
+    const float gx = fmaxf(0.0f, fmaxf(t.xlo - s.xhi, s.xlo - t.xhi));
+    const float gy = fmaxf(0.0f, fmaxf(t.ylo - s.yhi, s.ylo - t.yhi));
+    const float d2 = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
+    const float c = fmaxf(fmaxf(t.cmax, s.cmax), k.Lh);
+    const float hh = t.hmax + s.hmax;
+    const float ext = fmaxf(fmaxf(s.xhi - s.xlo, s.yhi - s.ylo), s.zhi - s.zlo);
+    return d2 > 1.01f * hh * hh && k.simple_ratio2 * d2 >= 1.01f * c * c && d2 >= k.simple_ext2 * ext * ext;   // false for NaN / padding
+}
+
 // Same grid / decomposition / acc layout as pair_fp64_sym_kernel.
 template <int NC>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_MIXED_MINBLOCKS)
@@ -276,7 +366,8 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
                       const double *__restrict__ hs,
                       const double *__restrict__ tile_hmax, int n_pad, int n_tiles,
                       int tiles_per_chunk, int ncut_rt, MixedConsts k, PairConsts kd,
-                      const DevFlags *__restrict__ flags, double *__restrict__ acc)
+                      const DevFlags *__restrict__ flags, double *__restrict__ acc,
+                      unsigned long long *__restrict__ pass_stats)
 {
     __shared__ SymSmem sm;
     if (need_general_path(flags, kd.halfL)) {         // the fp64 general path (xy, zm, hs are only read here)
@@ -287,7 +378,7 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
     const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
-    float4 *s_hi = reinterpret_cast<float4 *>(sm.src), *s_lo = s_hi + PAIR_THREADS;
+    float4 *s_hi = reinterpret_cast<float4 *>(sm.src), *s_lo = s_hi + PAIR_THREADS, *s_rel = s_lo + PAIR_THREADS;
     float (*s_b)[3][PAIR_THREADS] = reinterpret_cast<float (*)[3][PAIR_THREADS]>(sm.b);
 
     // gridDim.z == 4 (small N): CTA z takes source sub-tile z only (see pair_fp64_sym_kernel)
@@ -313,12 +404,25 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
     ti2.yl = make_float2(ti[0].yl, ti[1].yl); ti2.zl = make_float2(ti[0].zl, ti[1].zl);
     ti2.h = make_float2(ti[0].h, ti[1].h);    ti2.m = make_float2(ti[0].m, ti[1].m);
     ti2.mL = make_float2(ti[0].mL, ti[1].mL);
+    // bounding box of this warp's 64 targets, and (per staged tile) of each 32-source sub-tile
+    const MixBox tbox = box_warp(box_join(box_of(ti[0].xh, ti[0].yh, ti[0].zh, ti[0].h),
+                                          box_of(ti[1].xh, ti[1].yh, ti[1].zh, ti[1].h)));
+    __shared__ MixBox s_box[PAIR_THREADS / 32];
+    unsigned n_simple = 0, n_pass = 0;                 // two-way ring passes of this warp: SIMPLE / all
 
     for (int t = t0; t < t1; ++t) {
         const int j = t * PAIR_THREADS + threadIdx.x;
         __syncthreads();
-        s_hi[threadIdx.x] = f_hi[j];
-        s_lo[threadIdx.x] = f_lo[j];
+        {
+            const float4 vh = f_hi[j], vl = f_lo[j];
+            s_hi[threadIdx.x] = vh;
+            s_lo[threadIdx.x] = vl;
+            const MixBox sb = box_warp(box_of(vh.x, vh.y, vh.z, vl.w));
+            if (lane == 0) s_box[w] = sb;
+            // offsets from the sub-tile's centre as single floats (SIMPLE passes)
+            const float ox = 0.5f * (sb.xlo + sb.xhi), oy = 0.5f * (sb.ylo + sb.yhi), oz = 0.5f * (sb.zlo + sb.zhi);
+            s_rel[threadIdx.x] = make_float4((vh.x - ox) + vl.x, (vh.y - oy) + vl.y, (vh.z - oz) + vl.z, vh.w);
+        }
         __syncthreads();
         int soft_bits[SYM_R];
         {
@@ -335,7 +439,17 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
             const float4 *sh = s_hi + js * 32, *sl = s_lo + js * 32;
             if (t >= tb + SYM_R) {
                 float2 a2[4], b2x, b2y, b2z;
-                ring_subtile_f32x2<NC>(ti2, soft_bits, sh, sl, lane, k, ncut_rt, a2, b2x, b2y, b2z);
+                float zshift;
+                n_pass += 1;
+                const MixBox sb = s_box[js];
+                if (pass_is_simple(tbox, sb, k, zshift)) {              // warp-uniform
+                    n_simple += 1;
+                    ring_subtile_f32x2<NC, true>(ti2, soft_bits, sh, sl, lane, k, ncut_rt, a2, b2x, b2y, b2z,
+                                                 s_rel + js * 32, 0.5f * (sb.xlo + sb.xhi), 0.5f * (sb.ylo + sb.yhi),
+                                                 0.5f * (sb.zlo + sb.zhi), zshift);
+                } else {
+                    ring_subtile_f32x2<NC, false>(ti2, soft_bits, sh, sl, lane, k, ncut_rt, a2, b2x, b2y, b2z);
+                }
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     A[0][c] += (double)a2[c].x;
@@ -380,6 +494,10 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
 #pragma unroll
         for (int c = 0; c < 4; ++c) atomicAdd(acc + (size_t)c * n_pad + i, A[r][c]);
+    }
+    if (lane == 0 && n_pass != 0) {                    // cumulative statistics (steps_cyl_pass_stats)
+        atomicAdd(pass_stats, (unsigned long long)n_simple);
+        atomicAdd(pass_stats + 1, (unsigned long long)n_pass);
     }
 }
 

@@ -59,6 +59,7 @@ struct steps_cyl_ctx {
     int n_pow2 = 0;
     int *perm = nullptr;                           // packed slot -> caller index
     unsigned long long *order_keys = nullptr, *rmax_bits = nullptr;
+    unsigned long long *pass_stats = nullptr;      // mixed kernel: SIMPLE / all ring passes since init
     GraphSlot gslot[2];                            // STEPS_FLAG_GRAPH: one captured evaluation per flag-block parity
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
@@ -263,7 +264,7 @@ void launch_pair_mixed_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
     dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
     pair_mixed_sym_kernel<NC><<<grid, PAIR_THREADS, 0, s>>>(c->f_hi, c->f_lo, c->xy, c->zm, c->hs, c->tile_hmax,
                                                            c->n_pad, c->n_tiles, c->sym_tiles_per_chunk,
-                                                           c->p.n_cut, c->mc, c->kc, c->cur_flags, c->part);
+                                                           c->p.n_cut, c->mc, c->kc, c->cur_flags, c->part, c->pass_stats);
 }
 
 // EWALD_TABLE + DETERMINISTIC: one launch per round (pair_table_round.cuh).
@@ -751,6 +752,10 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->mc.Lh = (float)L;
     ctx->mc.Ll = (float)(L - (double)ctx->mc.Lh);
     ctx->mc.halfL = (float)(0.5 * L);
+    // SIMPLE ring passes of the mixed kernel (pair_mixed_sym.cuh: pass_is_simple): box distance d >= c / 8 and
+    // d >= (source box extent) / 2 -- measured at configs 1-3: parity as without them, 87 % of the passes at N = 1 M
+    ctx->mc.simple_ratio2 = 64.0f;
+    ctx->mc.simple_ext2 = 0.25f;
     for (int n = 0; n <= MAX_NCUT_TABLE; ++n) {
         const double nL = (double)n * L;
         ctx->kc.c2nL[n] = 2.0 * nL;
@@ -771,6 +776,8 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
     A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 5)));
+    A(dev_alloc(&ctx->pass_stats, 2));
+    if (rc == STEPS_OK) A(cudaMemset(ctx->pass_stats, 0, 2 * sizeof(unsigned long long)));
     A(dev_alloc(&ctx->flags, 3));                   // two alternating blocks + the sticky h <= 0 word
     A(dev_alloc(&ctx->peak_out, 1));
     A(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
@@ -833,6 +840,16 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         A(dev_alloc(&ctx->rmax_bits, 1));
         if (rc != STEPS_OK) return fail(rc);
     }
+    if (!ctx->use_order && pp.precision == STEPS_PREC_MIXED) {
+        // mixed precision: spatially ordered packed arrays let most ring passes take the plain-float form
+        // (pair_mixed_sym.cuh: pass_is_simple)
+        ctx->use_order = true;
+        ctx->n_pow2 = 1024;
+        while (ctx->n_pow2 < ctx->n) ctx->n_pow2 <<= 1;
+        A(dev_alloc(&ctx->perm, (size_t)ctx->n));
+        A(dev_alloc(&ctx->order_keys, (size_t)ctx->n_pow2));
+        A(dev_alloc(&ctx->rmax_bits, 1));
+    }
     A(cudaMemset(ctx->flags, 0, 3 * sizeof(DevFlags)));
     if (rc != STEPS_OK) return fail(rc);
     ctx->bad_h_sticky = reinterpret_cast<int *>(ctx->flags + 2);
@@ -850,7 +867,7 @@ void steps_cyl_destroy(steps_cyl_ctx *c)
         if (g.graph) cudaGraphDestroy(g.graph);
     }
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->perm); cudaFree(c->order_keys); cudaFree(c->rmax_bits); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
+    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->perm); cudaFree(c->order_keys); cudaFree(c->rmax_bits); cudaFree(c->pass_stats); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -1065,6 +1082,18 @@ const char *steps_cyl_strerror(int code)
 const char *steps_cyl_last_cuda_error(steps_cyl_ctx *ctx) { return ctx ? ctx->cuda_msg : ""; }
 
 const char *steps_cyl_pair_kernel_name(steps_cyl_ctx *ctx) { return ctx ? ctx->kernel_name : ""; }
+
+int steps_cyl_pass_stats(steps_cyl_ctx *ctx, void *cuda_stream, uint64_t *simple, uint64_t *total)
+{
+    if (!ctx || !simple || !total) return STEPS_EINVAL;
+    ON_DEVICE(ctx);
+    CK(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    unsigned long long v[2] = {0, 0};
+    CK(cudaMemcpy(v, ctx->pass_stats, sizeof v, cudaMemcpyDeviceToHost));
+    *simple = v[0];
+    *total = v[1];
+    return STEPS_OK;
+}
 
 int64_t steps_cyl_launch_count(steps_cyl_ctx *ctx) { return ctx ? ctx->launches : 0; }
 

@@ -130,33 +130,47 @@ def analyse(ins):
         cands.append((arith, lo, hi, bool(inner)))
     if not cands:
         return None
+
+    def tally_loop(lo, hi):
+        b = body(lo, hi)
+        # blocks a forward conditional branch inside the loop can skip; one that ends in a CALL (the noinline
+        # spline of Eq. 3 behind its pre-test) is the slow path and is tallied apart, any other (e.g. the table
+        # gathers only lanes inside rho_max take) counts as executed
+        skip = []
+        for a, pred, t in b:
+            m = _BRA.search(t)
+            if m and t.startswith("BRA") and pred is not None:
+                tgt = int(m.group(1), 16)
+                if a < tgt <= hi:
+                    skip.append((a, tgt, any(t2.startswith("CALL") for a2, _, t2 in b if a < a2 < tgt)))
+        main, skipped = Counter(), Counter()
+        for a, pred, t in b:
+            op = t.split()[0]
+            key = _base(t)
+            slow = any(s < a < e and call for s, e, call in skip)
+            if key in ("DFMA", "DMUL", "DADD") and not slow:
+                # distinct 64-bit REGISTER sources (not RZ / uniform registers / constants / immediates): an FP64
+                # instruction with three of them issues over three cycles instead of two (measured)
+                srcs = set(re.findall(r"(?<![U\w])R(\d+)", t.split(",", 1)[1] if "," in t else ""))
+                if len(srcs) >= 3:
+                    main["fp64_three_reg_sources"] += 1
+            if key == "MUFU":
+                key = op                      # MUFU.RSQ / MUFU.RSQ64H / MUFU.RCP ...
+            (skipped if slow else main)[key] += 1
+        return main, skipped
+
     _, lo, hi, nested = max(cands)
-    b = body(lo, hi)
-    # blocks a forward conditional branch inside the loop can skip; one that ends in a CALL (the noinline
-    # spline of Eq. 3 behind its pre-test) is the slow path and is tallied apart, any other (e.g. the table
-    # gathers only lanes inside rho_max take) counts as executed
-    skip = []
-    for a, pred, t in b:
-        m = _BRA.search(t)
-        if m and t.startswith("BRA") and pred is not None:
-            tgt = int(m.group(1), 16)
-            if a < tgt <= hi:
-                skip.append((a, tgt, any(t2.startswith("CALL") for a2, _, t2 in b if a < a2 < tgt)))
-    main, skipped = Counter(), Counter()
-    for a, pred, t in b:
-        op = t.split()[0]
-        key = _base(t)
-        if key in ("DFMA", "DMUL", "DADD") and not any(s < a < e and call for s, e, call in skip):
-            # distinct 64-bit REGISTER sources (not RZ / uniform registers / constants / immediates): an FP64
-            # instruction with three of them issues over three cycles instead of two (measured)
-            srcs = set(re.findall(r"(?<![U\w])R(\d+)", t.split(",", 1)[1] if "," in t else ""))
-            if len(srcs) >= 3:
-                main["fp64_three_reg_sources"] += 1
-        if key == "MUFU":
-            key = op                      # MUFU.RSQ / MUFU.RSQ64H / MUFU.RCP ...
-        slow = any(s < a < e and call for s, e, call in skip)
-        (skipped if slow else main)[key] += 1
-    return lo, hi, main, skipped, nested
+    main, skipped = tally_loop(lo, hi)
+    # variants of the pair loop: other candidate loops with the same rsqrt and shuffle counts (same pairs per
+    # iteration), e.g. the SIMPLE ring pass of the mixed kernel; heaviest first, the main loop included
+    def sig(c):
+        return (sum(v for k, v in c.items() if k.startswith("MUFU")), c.get("SHFL", 0))
+    variants = []
+    for arith, l2, h2, _ in sorted(cands, reverse=True):
+        m2, _s2 = tally_loop(l2, h2)
+        if sig(m2) == sig(main):
+            variants.append((l2, h2, m2))
+    return lo, hi, main, skipped, nested, variants
 
 
 def derive(kind_counts):
@@ -189,13 +203,16 @@ def tally(lib_path=LIB):
         res = analyse(funcs[mangled])
         if res is None:
             continue
-        lo, hi, main, skipped, nested = res
+        lo, hi, main, skipped, nested, variants = res
         inter = INTERACTIONS[fam]
         d = derive(main)
         kernels[short] = {
             "loop": ["0x%04x" % lo, "0x%04x" % hi], "interactions_per_iteration": inter, "nested": nested,
             "mainline": dict(sorted(main.items())), "slowpath": dict(sorted(skipped.items())),
             "per_interaction": {k: v / inter for k, v in d.items()},
+            # loops with the same pairs per iteration, heaviest first ([0] is the main loop)
+            "variants": [{"loop": ["0x%04x" % l2, "0x%04x" % h2],
+                          "per_interaction": {k: v / inter for k, v in derive(m2).items()}} for l2, h2, m2 in variants],
         }
     return {"library": os.path.basename(lib_path), "tool": "cuobjdump -sass", "kernels": kernels}
 
