@@ -840,9 +840,12 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
         A(dev_alloc(&ctx->rmax_bits, 1));
         if (rc != STEPS_OK) return fail(rc);
     }
-    if (!ctx->use_order && pp.precision == STEPS_PREC_MIXED) {
-        // mixed precision: spatially ordered packed arrays let most ring passes take the plain-float form
-        // (pair_mixed_sym.cuh: pass_is_simple)
+    if (!ctx->use_order && ctx->use_sym && pp.precision == STEPS_PREC_MIXED && ctx->n >= 16384) {
+        // mixed image-sum kernel: with spatially ordered packed arrays most ring passes are between far-apart groups
+        // and take the SIMPLE form (pair_mixed_sym.cuh: pass_is_simple); at small n the groups are too extended for
+        // that and the sort would only cost latency.  The fp64 image-sum kernel stays in caller order: measured, the
+        // analogous far-pass form gains nothing there (FP64-issue bound either way), and summing the sources in
+        // spatial order costs cancellation accuracy (1e-14 -> 1e-12 for core particles, kappa ~ 1e3).
         ctx->use_order = true;
         ctx->n_pow2 = 1024;
         while (ctx->n_pow2 < ctx->n) ctx->n_pow2 <<= 1;
