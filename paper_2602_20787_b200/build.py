@@ -20,7 +20,8 @@ SASSMIX = os.path.join(HERE, "libsteps_cyl.sassmix.json")
 
 def _deps() -> list:
     """Everything the library is compiled from: all of csrc/ plus the public header (content-hashed)."""
-    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h")))
+    files = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)
+                   if f.endswith((".cu", ".cuh", ".h")) and not f.startswith("ubench_"))
     return files + [os.path.join(os.path.dirname(HERE), "include", "steps_cyl.h"),
                     os.path.join(HERE, "sassmix.py")]
 

@@ -154,6 +154,8 @@ def analyse(ins):
                 srcs = set(re.findall(r"(?<![U\w])R(\d+)", t.split(",", 1)[1] if "," in t else ""))
                 if len(srcs) >= 3:
                     main["fp64_three_reg_sources"] += 1
+                elif len(srcs) == 2:
+                    main["fp64_two_reg_sources"] += 1
             if key == "MUFU":
                 key = op                      # MUFU.RSQ / MUFU.RSQ64H / MUFU.RCP ...
             (skipped if slow else main)[key] += 1
@@ -184,9 +186,11 @@ def derive(kind_counts):
     fp32_issue = sum(c.get(k, 0) for k in FP32_OPS)
     mufu = sum(v for k, v in c.items() if k.startswith("MUFU"))
     conv = sum(v for k, v in c.items() if k in ("F2F", "F2I", "I2F", "F2FP"))
-    three = c.get("fp64_three_reg_sources", 0)
-    return dict(fp64_three_reg=three, fp64_issue_cycles=2 * fp64_instr + three, fp64_instr=fp64_instr, fp64_flops=fp64_flops, fp32_ops=fp32_ops, fp32_flops=fp32_flops,
-                fp32_issue=fp32_issue, mufu=mufu, conv=conv, total=sum(v for k, v in c.items() if k != "fp64_three_reg_sources"))
+    three, two = c.get("fp64_three_reg_sources", 0), c.get("fp64_two_reg_sources", 0)
+    # issue cycles of the FP64 instructions alone, with the measured costs per operand form (ubench_fp64_pipe.cu:
+    # 2.0 cycles with at most one register source, 2.1 with two, 3.0 with three distinct ones)
+    return dict(fp64_three_reg=three, fp64_two_reg=two, fp64_issue_cycles=2.0 * fp64_instr + 0.1 * two + 1.0 * three, fp64_instr=fp64_instr, fp64_flops=fp64_flops, fp32_ops=fp32_ops, fp32_flops=fp32_flops,
+                fp32_issue=fp32_issue, mufu=mufu, conv=conv, total=sum(v for k, v in c.items() if not k.startswith("fp64_t")))
 
 
 def tally(lib_path=LIB):
