@@ -122,10 +122,15 @@ typedef struct {
     double  tab_rho_max;    /* radial extent of the table; beyond it the pair force is the line-mass
                                term -2 G m/(Lz rho) e_rho (reading T2)            [5 Lz]              */
     int32_t interp;         /* STEPS_INTERP_CIC or STEPS_INTERP_TSC                    */
-    int32_t tab_fp32;       /* 0: table nodes in double, read from global memory;  1: nodes rounded to
-                               float and held in shared memory (the paper's (5,12) Ewald sum is itself
-                               single-precision accurate); needs nrho*nz*8 B + 56 KB of
-                               shared memory per SM (144 x 128 fits), else STEPS_EUNSUPPORTED          */
+    int32_t tab_fp32;       /* precision tier of the table (with precision = STEPS_PREC_FP64; MIXED implies 1):
+                               0: nodes in double, interpolated in double -- the fp64 contract (<= 1e-10 per particle
+                                  against the same table interpolated by the definition);
+                               1: "fp64 pairs, fp32 table": nodes rounded to float, held in shared memory, their
+                                  weighted sum taken in fp32, everything else double.  Contract: max <= 2e-6, median
+                                  <= 5e-8 per particle against the same float nodes interpolated in double (<= 4 float
+                                  roundings of each pair's D; the paper's (5,12) Ewald sum behind the nodes is itself
+                                  single-precision accurate).  Needs nrho*nz*8 B + 56 KB of shared
+                                  memory per SM (144 x 128 fits), else STEPS_EUNSUPPORTED                     */
 } steps_cyl_params;
 
 /* Validate `p`, select the device, allocate scratch for n particles and build the constant
