@@ -63,6 +63,9 @@ struct BgParams {
     const QuadNode *nodes;
 };
 struct KickParams { double inv_a3, H, dt; };
+// Single-writer slabs of the deterministic symmetric kernel (pair_fp64_sym.cuh, SLAB): rows = CTA rows of the pair
+// kernel (tr target tiles each), then chunks x split target-side slabs; tpc = source tiles per chunk.  rows == 0: off.
+struct SlabLayout { int rows, tr, tpc, chunks, split; };
 
 template <int LANES> struct OnStep {
     static constexpr int kParticlesPerBlock = (LANES == 32) ? 8 : PAIR_THREADS;
@@ -192,7 +195,7 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
                 double *__restrict__ gx, double *__restrict__ gy, double *__restrict__ gz,
                 const double *__restrict__ x, const double *__restrict__ y,
                 double *__restrict__ vx, double *__restrict__ vy, double *__restrict__ vz,
-                BgParams bg, KickParams kp, const int *__restrict__ perm)
+                BgParams bg, KickParams kp, const int *__restrict__ perm, SlabLayout sl)
 {
     const int lane = threadIdx.x & 31;
     const int i = (LANES == 32) ? blockIdx.x * OnStep<LANES>::kParticlesPerBlock + (threadIdx.x >> 5)
@@ -208,6 +211,25 @@ poststep_kernel(const double *__restrict__ part, int n, int n_pad, int n_slabs, 
     }
     if (LANES == 32 && lane != 0) return;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (sl.rows > 0) {
+        // the slots of particle i that were written, in fixed order: source-side sums from every CTA row at or
+        // below its tile's row, target-side sums from every non-empty CTA (chunk, sub-tile) of its own row
+        const size_t slab = 3 * (size_t)n_pad;
+        const int tile = i / PAIR_THREADS, row = tile / sl.tr;
+        for (int bx = 0; bx <= row; ++bx) {
+            const double *p = part + (size_t)bx * slab + i;
+            a0 += p[0];
+            a1 += p[(size_t)n_pad];
+            a2 += p[2 * (size_t)n_pad];
+        }
+        for (int c = (row * sl.tr) / sl.tpc; c < sl.chunks; ++c)
+            for (int z = 0; z < sl.split; ++z) {
+                const double *p = part + ((size_t)sl.rows + (size_t)c * sl.split + z) * slab + i;
+                a0 += p[0];
+                a1 += p[(size_t)n_pad];
+                a2 += p[2 * (size_t)n_pad];
+            }
+    } else
     for (int c = 0; c < n_slabs; ++c) {
         const double *p = part + (size_t)c * 4 * n_pad + i;
         a0 += p[0];

@@ -141,28 +141,37 @@ struct SymSmem {
 // grid = (n_tiles / SYM_R, chunks).  CTA (bi, c): target tiles SYM_R*bi + r (lane holds particle
 // tid of each), source tiles [c*tpc, (c+1)*tpc) from SYM_R*bi on.
 // GENERAL: the same decomposition with the general pair law (ring_subtile<..., GENERAL>).
-template <int NC, bool O2, bool GENERAL, class KC>
+// SLAB (STEPS_FLAG_DETERMINISTIC up to N = 131 072): instead of atomics every sum goes to a slot with exactly one
+// writer -- source-side sums of CTA row bx to slab bx (each (row, source tile) is handled by one CTA), target-side
+// sums of CTA (bx, c, z) to slab gridDim.x + c * gridDim.z + z -- and poststep_kernel adds the slots that were
+// written (a rule on indices, no zeroing) in fixed order: bit-reproducible at the speed of the atomic kernel.
+template <int NC, bool O2, bool GENERAL, int TR, bool SLAB, class KC>
 __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                                          const double *__restrict__ hs, const double *__restrict__ tile_hmax,
                                          int n_pad, int n_tiles, int tiles_per_chunk, int ncut_rt,
                                          const KC &k, double *__restrict__ acc, SymSmem &sm)
 {
-    const int tb = blockIdx.x * SYM_R;                       // first target tile of this CTA
+    const int tb = blockIdx.x * TR;                       // first target tile of this CTA
     const int t0 = max(blockIdx.y * tiles_per_chunk, tb);
     const int t1 = min((blockIdx.y + 1) * tiles_per_chunk, n_tiles);
     if (t0 >= t1) return;
     SymSrc *s_src = sm.src;
     double (*s_b)[3][PAIR_THREADS] = sm.b;
+    double *slab_src = acc, *slab_tgt = acc;
+    if (SLAB) {
+        slab_src = acc + (size_t)blockIdx.x * 3 * n_pad;
+        slab_tgt = acc + ((size_t)gridDim.x + (size_t)blockIdx.y * gridDim.z + blockIdx.z) * 3 * n_pad;
+    }
 
     // gridDim.z == 4 (small N: fewer tile pairs than the GPU has schedulers): CTA z takes source sub-tile z only
     const bool split = gridDim.z == PAIR_THREADS / 32;
     const int js0 = split ? blockIdx.z : 0, js1 = split ? blockIdx.z + 1 : PAIR_THREADS / 32;
     const bool mine = (int)threadIdx.x >= js0 * 32 && (int)threadIdx.x < js1 * 32;   // sources this CTA takes
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    SymTgt ti[SYM_R];
-    double a[SYM_R][3];
+    SymTgt ti[TR];
+    double a[TR][3];
 #pragma unroll
-    for (int r = 0; r < SYM_R; ++r) {
+    for (int r = 0; r < TR; ++r) {
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
         const double2 pi = xy[i], qi = zm[i];
         ti[r].x = pi.x; ti[r].y = pi.y; ti[r].z = qi.x; ti[r].m = qi.y; ti[r].h = hs[i];
@@ -179,11 +188,11 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
             s_src[threadIdx.x] = v;
         }
         __syncthreads();
-        int soft_hi[SYM_R];
+        int soft_hi[TR];
         {
             const double hm = tile_hmax[t];
 #pragma unroll
-            for (int r = 0; r < SYM_R; ++r) {
+            for (int r = 0; r < TR; ++r) {
                 const double b = ti[r].h + hm;
                 soft_hi[r] = hi32(b * b);
             }
@@ -192,15 +201,15 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
         for (int js = js0; js < js1; ++js) {
             double bx = 0.0, by = 0.0, bz = 0.0;
             const SymSrc *sub = s_src + js * 32;
-            if (t >= tb + SYM_R) {
+            if (t >= tb + TR) {
                 // off-diagonal tile: every target of the CTA meets every source, both ways
-                ring_subtile<NC, SYM_R, true, O2, GENERAL, KC>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
+                ring_subtile<NC, TR, true, O2, GENERAL, KC>(ti, soft_hi, sub, lane, k, ncut_rt, a, bx, by, bz);
             } else {
                 // one of the CTA's own tiles: target tile tb + r meets source tile t only if
                 // t >= tb + r; in its own tile (t == tb + r) warp w takes sub-tiles js > w both
                 // ways, js == w target-side only, and leaves js < w to the warp that owns them.
 #pragma unroll
-                for (int r = 0; r < SYM_R; ++r) {
+                for (int r = 0; r < TR; ++r) {
                     if (tb + r > t) continue;
                     const SymTgt (&t1r)[1] = reinterpret_cast<const SymTgt (&)[1]>(ti[r]);
                     const int (&s1r)[1] = reinterpret_cast<const int (&)[1]>(soft_hi[r]);
@@ -224,27 +233,37 @@ __device__ __forceinline__ void sym_body(const double2 *__restrict__ xy, const d
             double v = s_b[0][c][threadIdx.x];
 #pragma unroll
             for (int ww = 1; ww < PAIR_THREADS / 32; ++ww) v += s_b[ww][c][threadIdx.x];
-            if (mine && v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
+            if (SLAB) {
+                if (mine) slab_src[(size_t)c * n_pad + j] = -v;
+            } else {
+                if (mine && v != 0.0) atomicAdd(acc + (size_t)c * n_pad + j, -v);
+            }
         }
     }
 #pragma unroll
-    for (int r = 0; r < SYM_R; ++r) {
+    for (int r = 0; r < TR; ++r) {
         const int i = (tb + r) * PAIR_THREADS + threadIdx.x;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
+        for (int c = 0; c < 3; ++c) {
+            if (SLAB) slab_tgt[(size_t)c * n_pad + i] = a[r][c];
+            else atomicAdd(acc + (size_t)c * n_pad + i, a[r][c]);
+        }
     }
 }
 
 // The general path of the symmetric kernels (fp64 and mixed), out of line: it costs the fast path no registers.
+template <int TR, bool SLAB = false>
 __device__ __noinline__ void sym_body_general(const double2 *xy, const double2 *zm, const double *hs,
                                               const double *tile_hmax, int n_pad, int n_tiles,
                                               int tiles_per_chunk, int ncut_rt, WrapConsts k,
                                               double *acc, SymSmem &sm)
 {
-    sym_body<0, false, true>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+    sym_body<0, false, true, TR, SLAB>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
 }
 
-template <int NC, bool O2>
+// TR = target tiles per CTA: SYM_R = 2 in general; 1 in the small-N split mode (gridDim.z = 4), where the kernel
+// time is one CTA's critical path -- a CTA of the diagonal then walks one single-target ring pass instead of two.
+template <int NC, bool O2, int TR = SYM_R, bool SLAB = false>
 __global__ void __launch_bounds__(PAIR_THREADS, STEPS_SYM_MINBLOCKS)
 pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__ zm,
                      const double *__restrict__ hs, const double *__restrict__ tile_hmax,
@@ -253,10 +272,10 @@ pair_fp64_sym_kernel(const double2 *__restrict__ xy, const double2 *__restrict__
 {
     __shared__ SymSmem sm;
     if (need_general_path(flags, k.halfL)) {          // decided on the device: no host synchronisation
-        sym_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+        sym_body_general<TR, SLAB>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
         return;
     }
-    sym_body<NC, O2, false>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
+    sym_body<NC, O2, false, TR, SLAB>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, k, acc, sm);
 }
 
 // ---------------------------------------------------------------------------------------------

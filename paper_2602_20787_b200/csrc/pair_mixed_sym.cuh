@@ -371,7 +371,7 @@ pair_mixed_sym_kernel(const float4 *__restrict__ f_hi, const float4 *__restrict_
 {
     __shared__ SymSmem sm;
     if (need_general_path(flags, kd.halfL)) {         // the fp64 general path (xy, zm, hs are only read here)
-        sym_body_general(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, kd, acc, sm);
+        sym_body_general<SYM_R>(xy, zm, hs, tile_hmax, n_pad, n_tiles, tiles_per_chunk, ncut_rt, kd, acc, sm);
         return;
     }
     const int tb = blockIdx.x * SYM_R;

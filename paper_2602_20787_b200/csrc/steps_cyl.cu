@@ -40,6 +40,9 @@ struct steps_cyl_ctx {
     int sym_chunks, sym_tiles_per_chunk;          // decomposition of the symmetric kernel
     bool use_sym;                                 // !STEPS_FLAG_DETERMINISTIC
     int sym_split = 1;                            // gridDim.z of the symmetric image-mode kernels (1 or 4)
+    bool sym_small = false;                       // fp64 image mode at small N: one target tile per CTA (TR = 1)
+    bool use_slabs = false;                       // DETERMINISTIC fp64 image mode up to N = 131072: single-writer slabs
+    int sym_tr() const { return sym_small ? 1 : SYM_R; }
     int round_split = 1;                          // gridDim.y of the image-mode round kernels (1 or 4)
     bool use_rounds;                              // DETERMINISTIC: round-scheduled symmetric kernels
     int sm_count;
@@ -201,17 +204,31 @@ void launch_pair_fp64_nc(steps_cyl_ctx *c, cudaStream_t s)
 template <int NC>
 void launch_pair_sym_nc(steps_cyl_ctx *c, cudaStream_t s)
 {
-    dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
-    if (c->p.flags & STEPS_FLAG_FAR_ORDER2)
-        pair_fp64_sym_kernel<NC, true><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
-                                                                    c->n_pad, c->n_tiles,
-                                                                    c->sym_tiles_per_chunk, c->p.n_cut,
-                                                                    c->kc, c->cur_flags, c->part);
-    else
-        pair_fp64_sym_kernel<NC, false><<<grid, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax,
-                                                                     c->n_pad, c->n_tiles,
-                                                                     c->sym_tiles_per_chunk, c->p.n_cut,
-                                                                     c->kc, c->cur_flags, c->part);
+    const bool o2 = (c->p.flags & STEPS_FLAG_FAR_ORDER2) != 0;
+#define SYM_LAUNCH(O2, TR, GRID)                                                                            \
+    pair_fp64_sym_kernel<NC, O2, TR><<<GRID, PAIR_THREADS, 0, s>>>(c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, \
+                                                                  c->n_tiles, c->sym_tiles_per_chunk, c->p.n_cut, \
+                                                                  c->kc, c->cur_flags, c->part)
+    if (c->use_slabs) {
+        // DETERMINISTIC: the same kernel with single-writer slots instead of atomics
+        const dim3 grid(c->n_tiles / c->sym_tr(), c->sym_chunks, c->sym_split);
+        if (c->sym_small)
+            pair_fp64_sym_kernel<NC, false, 1, true><<<grid, PAIR_THREADS, 0, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->p.n_cut, c->kc,
+                c->cur_flags, c->part);
+        else
+            pair_fp64_sym_kernel<NC, false, SYM_R, true><<<grid, PAIR_THREADS, 0, s>>>(
+                c->xy, c->zm, c->hs, c->tile_hmax, c->n_pad, c->n_tiles, c->sym_tiles_per_chunk, c->p.n_cut, c->kc,
+                c->cur_flags, c->part);
+    } else if (c->sym_small) {
+        // small N: one target tile and one source sub-tile per CTA (the kernel time is one CTA's critical path)
+        const dim3 grid(c->n_tiles, c->sym_chunks, c->sym_split);
+        if (o2) SYM_LAUNCH(true, 1, grid); else SYM_LAUNCH(false, 1, grid);
+    } else {
+        const dim3 grid(c->n_tiles / SYM_R, c->sym_chunks, c->sym_split);
+        if (o2) SYM_LAUNCH(true, SYM_R, grid); else SYM_LAUNCH(false, SYM_R, grid);
+    }
+#undef SYM_LAUNCH
 }
 
 // Deterministic fp64 path: rounds of the symmetric evaluation, one launch each (pair_fp64_sym.cuh).
@@ -305,7 +322,8 @@ void launch_table_rounds(steps_cyl_ctx *c, cudaStream_t s)
 // The kernel launch_pair() selects, spelled as sassmix.py spells the template instances.
 void name_pair_kernel(steps_cyl_ctx *c)
 {
-    const bool mixed = c->p.precision == STEPS_PREC_MIXED, det = c->use_rounds, ord = !c->use_sym && !c->use_rounds;
+    const bool mixed = c->p.precision == STEPS_PREC_MIXED, det = c->use_rounds,
+               ord = !c->use_sym && !c->use_rounds && !c->use_slabs;
     const int nc = c->p.n_cut <= MAX_NCUT_UNROLLED ? c->p.n_cut : 0;
     char *o = c->kernel_name;
     const size_t cap = sizeof c->kernel_name;
@@ -316,12 +334,15 @@ void name_pair_kernel(steps_cyl_ctx *c)
     } else if (ord) {
         if (mixed) snprintf(o, cap, "pair_mixed_kernel<%d>", nc);
         else snprintf(o, cap, "pair_fp64_kernel<%d>", nc);
+    } else if (c->use_slabs) {
+        snprintf(o, cap, "pair_fp64_sym_kernel<%d,false,%d,true>", nc, c->sym_tr());
     } else if (det) {
         snprintf(o, cap, "pair_%s_round_kernel<%d,%s>", mixed ? "mixed" : "fp64", nc, c->round_split > 1 ? "true" : "false");
     } else if (mixed) {
         snprintf(o, cap, "pair_mixed_sym_kernel<%d>", nc);
     } else {
-        snprintf(o, cap, "pair_fp64_sym_kernel<%d,%s>", nc, (c->p.flags & STEPS_FLAG_FAR_ORDER2) ? "true" : "false");
+        snprintf(o, cap, "pair_fp64_sym_kernel<%d,%s,%d,false>", nc, (c->p.flags & STEPS_FLAG_FAR_ORDER2) ? "true" : "false",
+                 c->sym_tr());
     }
 }
 
@@ -373,7 +394,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<N>(c, s); \
         else if (mixed && c->use_rounds) launch_pair_mixed_rounds_nc<N>(c, s); \
         else if (mixed) launch_pair_mixed_nc<N>(c, s);           \
-        else if (c->use_sym) launch_pair_sym_nc<N>(c, s);        \
+        else if (c->use_sym || c->use_slabs) launch_pair_sym_nc<N>(c, s); \
         else if (c->use_rounds) launch_pair_rounds_nc<N>(c, s);  \
         else launch_pair_fp64_nc<N>(c, s);                       \
         break;
@@ -383,7 +404,7 @@ void launch_pair(steps_cyl_ctx *c, cudaStream_t s)
         if (mixed && c->use_sym) launch_pair_mixed_sym_nc<0>(c, s);
         else if (mixed && c->use_rounds) launch_pair_mixed_rounds_nc<0>(c, s);
         else if (mixed) launch_pair_mixed_nc<0>(c, s);
-        else if (c->use_sym) launch_pair_sym_nc<0>(c, s);
+        else if (c->use_sym || c->use_slabs) launch_pair_sym_nc<0>(c, s);
         else if (c->use_rounds) launch_pair_rounds_nc<0>(c, s);
         else launch_pair_fp64_nc<0>(c, s);
     }
@@ -451,11 +472,12 @@ struct PostVals {
     BgParams bg;
     KickParams kp;
     const int *perm;
-    void *args[19];
+    SlabLayout sl;
+    void *args[20];
     void bind()
     {
-        void *a[19] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &tile_hmax, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz,
-                       &bg, &kp, &perm};
+        void *a[20] = {&part, &n, &n_pad, &n_slabs, &G, &L, &fl_next, &tile_hmax, &gx, &gy, &gz, &x, &y, &vx, &vy, &vz,
+                       &bg, &kp, &perm, &sl};
         std::memcpy(args, a, sizeof a);
     }
 };
@@ -515,6 +537,11 @@ void fill_vals(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, PreVals 
     post.bg = pre.bg;
     post.kp = kick ? kick->k2 : none;
     pre.perm = post.perm = ctx->use_order ? ctx->perm : nullptr;
+    post.sl = {0, 1, 1, 1, 1};
+    if (ctx->use_slabs) {
+        post.sl = {ctx->n_tiles / ctx->sym_tr(), ctx->sym_tr(), ctx->sym_tiles_per_chunk, ctx->sym_chunks, ctx->sym_split};
+        pre.zero_rows = 0;
+    }
 }
 
 int enqueue_force_plain(steps_cyl_ctx *ctx, const ForceArgs &f, unsigned parity, bool timed, cudaStream_t s)
@@ -730,7 +757,18 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     ctx->n_pad = ctx->n_tiles * PAIR_THREADS;
     choose_chunks(ctx);
     ctx->use_sym = !(p->flags & (STEPS_FLAG_DETERMINISTIC | STEPS_FLAG_ORDERED_PAIRS));
+    ctx->sym_small = ctx->use_sym && ctx->sym_split > 1 && pp.precision == STEPS_PREC_FP64 &&
+                     pp.periodic_mode == STEPS_PERIODIC_IMAGES;
     ctx->use_rounds = (p->flags & STEPS_FLAG_DETERMINISTIC) && !(p->flags & STEPS_FLAG_ORDERED_PAIRS);
+    // DETERMINISTIC, fp64 image mode, N <= 131072: the symmetric kernel with single-writer slabs instead of atomics
+    // (n_tiles / TR + chunks x split slabs of 24 B x n_pad: 1.7 GB at the limit); above, and in the other modes, the
+    // round-scheduled kernels (within 3 % of the atomic ones from N ~ 260 000 up)
+    if (ctx->use_rounds && pp.precision == STEPS_PREC_FP64 && pp.periodic_mode == STEPS_PERIODIC_IMAGES &&
+        ctx->n <= 131072) {
+        ctx->use_rounds = false;
+        ctx->use_slabs = true;
+        ctx->sym_small = ctx->sym_split > 1;
+    }
 
     // small N: a round has n_tiles / 2 items of four warps; below ~1.5 warps per scheduler (measured break-even:
     // N ~ 260 000) split the items by source sub-tile
@@ -775,7 +813,13 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
     if (rc == STEPS_OK) A(cudaMemset(ctx->tile_hmax, 0, (size_t)ctx->n_tiles * sizeof(double)));
     A(dev_alloc(&ctx->f_hi, np));
     A(dev_alloc(&ctx->f_lo, np));
-    A(dev_alloc(&ctx->part, np * 4 * (size_t)std::max(ctx->n_chunks, 5)));
+    {
+        size_t part_doubles = np * 4 * (size_t)std::max(ctx->n_chunks, 5);
+        if (ctx->use_slabs)
+            part_doubles = std::max(part_doubles, np * 3 * ((size_t)ctx->n_tiles / ctx->sym_tr() +
+                                                           (size_t)ctx->sym_chunks * ctx->sym_split));
+        A(dev_alloc(&ctx->part, part_doubles));
+    }
     A(dev_alloc(&ctx->pass_stats, 2));
     if (rc == STEPS_OK) A(cudaMemset(ctx->pass_stats, 0, 2 * sizeof(unsigned long long)));
     A(dev_alloc(&ctx->flags, 3));                   // two alternating blocks + the sticky h <= 0 word

@@ -209,6 +209,8 @@ def tally(lib_path=LIB):
             continue
         lo, hi, main, skipped, nested, variants = res
         inter = INTERACTIONS[fam]
+        if fam == "pair_fp64_sym_kernel":        # <N_cut, FAR_ORDER2, target tiles per CTA>: 2 interactions per target
+            inter = 2 * int(short.rstrip(">").split(",")[2])
         d = derive(main)
         kernels[short] = {
             "loop": ["0x%04x" % lo, "0x%04x" % hi], "interactions_per_iteration": inter, "nested": nested,

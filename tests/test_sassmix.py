@@ -26,7 +26,8 @@ def every_selectable_kernel():
     """Every name steps_cyl_pair_kernel_name() can return (steps_cyl.cu: name_pair_kernel)."""
     names = []
     for nc in range(0, 9):
-        names += ["pair_fp64_sym_kernel<%d,%s>" % (nc, o2) for o2 in ("false", "true")]
+        names += ["pair_fp64_sym_kernel<%d,%s,%d,false>" % (nc, o2, tr) for o2 in ("false", "true") for tr in (1, 2)]
+        names += ["pair_fp64_sym_kernel<%d,false,%d,true>" % (nc, tr) for tr in (1, 2)]
         names += ["pair_fp64_round_kernel<%d,%s>" % (nc, sp) for sp in ("false", "true")]
         names += ["pair_mixed_round_kernel<%d,%s>" % (nc, sp) for sp in ("false", "true")]
         names += ["pair_fp64_kernel<%d>" % nc, "pair_mixed_kernel<%d>" % nc, "pair_mixed_sym_kernel<%d>" % nc]
@@ -49,7 +50,7 @@ def test_tally_covers_every_kernel_bench_can_select(mix):
 def test_default_fp64_kernel_count(mix):
     """pair_fp64_sym_kernel<5,false>: one ring step = 2 unordered pairs = 4 interactions; the design's count is
     108 FP64-pipe instructions per unordered pair; a regression in either direction shows."""
-    k = mix["kernels"]["pair_fp64_sym_kernel<5,false>"]
+    k = mix["kernels"]["pair_fp64_sym_kernel<5,false,2,false>"]
     assert k["interactions_per_iteration"] == 4 and not k["nested"]
     per_unordered = 2 * k["per_interaction"]["fp64_instr"]
     assert per_unordered <= 110, per_unordered
@@ -62,12 +63,12 @@ def test_default_fp64_kernel_count(mix):
 
 def test_per_image_cost_from_unrolled_instances(mix):
     from paper_2602_20787_b200 import sassmix
-    for fam, lo, hi in (("pair_fp64_sym_kernel<%d,false>", 8.0, 10.5), ("pair_fp64_kernel<%d>", 17.0, 21.0)):
+    for fam, lo, hi in (("pair_fp64_sym_kernel<%d,false,2,false>", 8.0, 10.5), ("pair_fp64_kernel<%d>", 17.0, 21.0)):
         d = (mix["kernels"][fam % 8]["per_interaction"]["fp64_instr"]
              - mix["kernels"][fam % 7]["per_interaction"]["fp64_instr"])
         assert lo <= d <= hi, (fam, d)              # two more images per pair evaluation
-    c20, how = sassmix.per_interaction(mix, "pair_fp64_sym_kernel<0,false>", 20)
-    c8, _ = sassmix.per_interaction(mix, "pair_fp64_sym_kernel<8,false>", 8)
+    c20, how = sassmix.per_interaction(mix, "pair_fp64_sym_kernel<0,false,2,false>", 20)
+    c8, _ = sassmix.per_interaction(mix, "pair_fp64_sym_kernel<8,false,2,false>", 8)
     assert "extrapolated" in how and c20["fp64_instr"] > 2.2 * c8["fp64_instr"]
 
 
