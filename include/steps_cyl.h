@@ -75,9 +75,11 @@ enum { STEPS_BG_FINITE = 0,            /* Eq. 9 with L = n_cut * Lz             
 enum { STEPS_FLAG_DETERMINISTIC = 1,   /* bit-reproducible results.  The default kernels evaluate every
                                           unordered pair once and add it to both particles with
                                           floating-point atomics (same terms, summation order varies from
-                                          run to run, ~1e-16).  With this flag both periodic modes
-                                          schedule the same evaluation in conflict-free rounds with
-                                          plain stores (~3 % slower)                                    */
+                                          run to run, ~1e-16).  With this flag the fp64 image mode up to
+                                          N = 131072 writes every sum to a slot with one writer and adds the
+                                          slots in fixed order (~4 % slower, 24 B x N x (N/256 + ~20) of
+                                          scratch); larger N and the other modes schedule the evaluation in
+                                          conflict-free rounds with plain stores (~3 % slower at N = 1M)     */
        STEPS_FLAG_FAR_ORDER2 = 2,      /* fp64 images mode, default kernel only: the rsqrt refinement of
                                           the FAR images (n != 0) drops its second-order term: 8 % faster,
                                           per-particle error <~ 2e-12 instead of ~1e-14 (bar: 1e-10)  */
