@@ -57,8 +57,9 @@ typedef enum {
     STEPS_ESOFT        = -2,  /* softening precondition violated: some h_i <= 0 (or NaN)                   */
     STEPS_ECUDA        = -3,  /* a CUDA runtime call failed (or no device present)                     */
     STEPS_ENOMEM       = -4,  /* host or device allocation failed                                      */
-    STEPS_EUNSUPPORTED = -5   /* a combination this build does not contain (EWALD_TABLE with
+    STEPS_EUNSUPPORTED = -5,  /* a combination this build does not contain (EWALD_TABLE with
                                  STEPS_FLAG_ORDERED_PAIRS, or a float table too large for shared memory) */
+    STEPS_ETOOBIG      = -6   /* steps_cyl_accel_noalloc only: n > STEPS_CYL_NOALLOC_MAX_N               */
 } steps_cyl_status;
 
 enum { STEPS_PERIODIC_IMAGES = 0,      /* Eq. 8, truncated image sum                                  */
@@ -163,6 +164,28 @@ int steps_cyl_accel_host(steps_cyl_ctx *ctx,
                          const double *x, const double *y, const double *z,
                          const double *m, const double *h,
                          double *gx, double *gy, double *gz);
+
+/* The same force evaluation as steps_cyl_accel -- g_i = sum_{j != i} m_j F_{S1xR2}(x_i - x_j, h_i + h_j), Eq. 1 +
+ * Eq. 8 + Eq. 3/4, fp64, truncated image sum with n_cut, the default symmetric kernel -- for callers that CANNOT
+ * ALLOCATE (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  It needs no
+ * context: it calls no cudaMalloc, cudaFree or other allocating routine, ever.  Its scratch (packed sources,
+ * accumulators, flags) is one static device array of STEPS_CYL_NOALLOC_MAX_N particle slots, 2.25 MiB, which every
+ * GPU that loads the library holds until the process exits.
+ * in : n, Lz, G, n_cut   as in steps_cyl_params;  x y z m h   device pointers on the CURRENT device, length n
+ * out: gx gy gz          device pointers, length n, overwritten.   Asynchronous on cuda_stream.
+ * Errors: EINVAL (NULL pointer, n < 1, Lz <= 0, n_cut < 1), ETOOBIG (n > STEPS_CYL_NOALLOC_MAX_N; nothing is
+ * launched), ECUDA.  h_i <= 0 is NOT reported by this call (there is no context to ask): the outputs are then
+ * unspecified.  2*max(h) > Lz/2 is handled as in steps_cyl_accel (general pair law, chosen on the device).
+ * - The first call on a device does the one-time set-up (address of the static array, SM count); make it outside
+ *   stream capture.  Later calls enqueue one 48-byte memset and three kernels, nothing else.
+ * - Every call on a device shares the one array, which keeps the last call's contents (what must start at zero
+ *   is cleared at the start of each call).  Two calls that OVERLAP on the GPU -- different streams, or graphs
+ *   replayed concurrently -- race on it: serialise them. */
+#define STEPS_CYL_NOALLOC_MAX_N ((int64_t)32768)
+int steps_cyl_accel_noalloc(int64_t n, double Lz, double G, int32_t n_cut,
+                            const double *x, const double *y, const double *z,
+                            const double *m, const double *h,
+                            double *gx, double *gy, double *gz, void *cuda_stream);
 
 /* Synchronise `cuda_stream` and return the deferred status of the calls enqueued so far on
  * this context (STEPS_OK, STEPS_ESOFT or STEPS_ECUDA); clears it. */

@@ -13,6 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsteps_cyl.so")
 
 STEPS_OK, STEPS_EINVAL, STEPS_ESOFT, STEPS_ECUDA, STEPS_ENOMEM, STEPS_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+STEPS_ETOOBIG = -6
+NOALLOC_MAX_N = 32768          # STEPS_CYL_NOALLOC_MAX_N
 PERIODIC_IMAGES, PERIODIC_EWALD_TABLE = 0, 1
 PREC_FP64, PREC_MIXED = 0, 1
 BG_FINITE, BG_INFINITE = 0, 1
@@ -27,7 +29,7 @@ EXPORTS = ["steps_cyl_init", "steps_cyl_destroy", "steps_cyl_accel", "steps_cyl_
            "steps_cyl_kdk_step_host",
            "steps_cyl_friedmann_step", "steps_cyl_friedmann_step_cpl", "steps_cyl_ewald_table", "steps_cyl_fp64_peak", "steps_cyl_last_pair_kernel_ms",
            "steps_cyl_strerror", "steps_cyl_last_cuda_error", "steps_cyl_launch_count",
-           "steps_cyl_pair_kernel_name", "steps_cyl_pass_stats"]
+           "steps_cyl_pair_kernel_name", "steps_cyl_pass_stats", "steps_cyl_accel_noalloc"]
 
 
 class Params(C.Structure):
@@ -65,6 +67,8 @@ def lib():
         L.steps_cyl_destroy.argtypes = [vp]
         L.steps_cyl_accel.restype = C.c_int
         L.steps_cyl_accel.argtypes = [vp] + [dp] * 8 + [vp]
+        L.steps_cyl_accel_noalloc.restype = C.c_int
+        L.steps_cyl_accel_noalloc.argtypes = [i64, d, d, C.c_int32] + [dp] * 8 + [vp]
         L.steps_cyl_accel_host.restype = C.c_int
         L.steps_cyl_accel_host.argtypes = [vp] + [dp] * 8
         L.steps_cyl_check.restype = C.c_int
@@ -151,6 +155,15 @@ def _host_ptr(a, n):
 def _stream():
     import torch
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def accel_noalloc(n, Lz, G, n_cut, x, y, z, m, h, gx, gy, gz):
+    """steps_cyl_accel_noalloc: context-free force evaluation that allocates nothing (n <= NOALLOC_MAX_N),
+    on torch's current device and stream (asynchronous); tensors are CUDA float64 of length n."""
+    ptrs = [_dev_ptr(t, int(n)) for t in (x, y, z, m, h, gx, gy, gz)]
+    rc = lib().steps_cyl_accel_noalloc(int(n), float(Lz), float(G), int(n_cut), *ptrs, _stream())
+    if rc:
+        raise StepsError(rc, lib().steps_cyl_strerror(rc).decode())
 
 
 class StepsCyl:

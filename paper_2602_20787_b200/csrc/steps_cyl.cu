@@ -696,6 +696,65 @@ int enqueue_background(steps_cyl_ctx *ctx, const double *x, const double *y, dou
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------
+// steps_cyl_accel_noalloc: one force evaluation (fp64, image mode, default symmetric kernel) that allocates
+// NOTHING -- for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+// that forbid it).  Everything steps_cyl_init would allocate for such an evaluation lives in ONE file-scope device
+// array of a fixed, modest size (every GPU that loads the library holds it until the process exits):
+//     xy[16 B] zm[16 B] hs[8 B] part[4 x 8 B] per particle slot, tile_hmax[8 B] per 128 slots, three flag blocks.
+// In HOST code the array's name is a host-side stand-in, not a device address, so its address is taken once per
+// device with cudaGetSymbolAddress (that device current) and only that pointer is ever handed to a kernel.
+// The array is shared by every call and keeps the last call's contents: what must start at zero (the flag blocks)
+// is cleared on the stream at the start of every call, the accumulator rows by prestep_kernel as in the ordinary path.
+constexpr int64_t kNoallocMaxN = STEPS_CYL_NOALLOC_MAX_N;
+static_assert(kNoallocMaxN % (SYM_R * PAIR_THREADS) == 0, "the limit is a whole number of CTA target groups");
+constexpr size_t kNoallocOffXy = 0;
+constexpr size_t kNoallocOffZm = kNoallocOffXy + sizeof(double2) * (size_t)kNoallocMaxN;
+constexpr size_t kNoallocOffHs = kNoallocOffZm + sizeof(double2) * (size_t)kNoallocMaxN;
+constexpr size_t kNoallocOffPart = kNoallocOffHs + sizeof(double) * (size_t)kNoallocMaxN;
+constexpr size_t kNoallocOffHmax = kNoallocOffPart + 4 * sizeof(double) * (size_t)kNoallocMaxN;
+constexpr size_t kNoallocOffFlags = kNoallocOffHmax + sizeof(double) * (size_t)(kNoallocMaxN / PAIR_THREADS);
+constexpr size_t kNoallocBytes = ((kNoallocOffFlags + 3 * sizeof(DevFlags) + 255) / 256) * 256;
+static_assert(kNoallocOffZm % 256 == 0 && kNoallocOffHs % 256 == 0 && kNoallocOffPart % 256 == 0 &&
+              kNoallocOffHmax % 256 == 0 && kNoallocOffFlags % 256 == 0, "every sub-array starts 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoallocBytes];      // 2.25 MiB per GPU
+
+namespace {
+
+struct NoallocDevice {
+    unsigned char *scratch = nullptr;      // DEVICE address of g_noalloc_scratch on this device
+    int sm_count = 0;
+    bool ready = false;
+};
+constexpr int kNoallocMaxDevices = 64;
+NoallocDevice g_noalloc_dev[kNoallocMaxDevices];
+std::mutex g_noalloc_mu;
+
+// Set-up, once per device, with that device current: the device address of the scratch array and the SM count.
+// Neither call allocates.  Returns cudaSuccess or the failing call's error.
+cudaError_t noalloc_setup(int dev, NoallocDevice **out)
+{
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    NoallocDevice &d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (ptr == nullptr || sms <= 0) return cudaErrorUnknown;
+        d.scratch = static_cast<unsigned char *>(ptr);
+        d.sm_count = sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return cudaSuccess;
+}
+
+}  // namespace
+
 extern "C" {
 
 int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
@@ -1113,6 +1172,70 @@ int steps_cyl_last_pair_kernel_ms(steps_cyl_ctx *ctx, float *ms)
     return STEPS_OK;
 }
 
+int steps_cyl_accel_noalloc(int64_t n, double Lz, double G, int32_t n_cut, const double *x, const double *y,
+                            const double *z, const double *m, const double *h, double *gx, double *gy,
+                            double *gz, void *cuda_stream)
+{
+    if (!x || !y || !z || !m || !h || !gx || !gy || !gz) return STEPS_EINVAL;
+    if (n < 1 || !(Lz > 0.0) || !std::isfinite(Lz) || !std::isfinite(G) || n_cut < 1 || n_cut > 1000000)
+        return STEPS_EINVAL;
+    if (n > kNoallocMaxN) return STEPS_ETOOBIG;          // before any CUDA call: the scratch array is fixed
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoallocMaxDevices) return STEPS_ECUDA;
+    NoallocDevice *nd = nullptr;
+    if (noalloc_setup(dev, &nd) != cudaSuccess) return STEPS_ECUDA;
+
+    // A throw-away context on the host stack whose scratch pointers all lie inside the static array; the launches
+    // are the ordinary ones (prestep_kernel, pair_fp64_sym_kernel, poststep_kernel through enqueue_force_plain).
+    steps_cyl_ctx c;
+    steps_cyl_ctx *ctx = &c;
+    c.cuda_msg[0] = 0;
+    c.kernel_name[0] = 0;
+    std::memset(&c.p, 0, sizeof c.p);
+    c.p.n = n; c.p.Lz = Lz; c.p.G = G; c.p.n_cut = n_cut; c.p.device = dev;
+    c.p.periodic_mode = STEPS_PERIODIC_IMAGES; c.p.precision = STEPS_PREC_FP64; c.p.background = STEPS_BG_FINITE;
+    c.sm_count = nd->sm_count;
+    c.n = (int)n;
+    c.n_tiles = SYM_R * ((c.n + SYM_R * PAIR_THREADS - 1) / (SYM_R * PAIR_THREADS));
+    c.n_pad = c.n_tiles * PAIR_THREADS;                  // <= kNoallocMaxN (a multiple of SYM_R * 128)
+    choose_chunks(ctx);
+    c.use_sym = true;
+    c.use_rounds = false;
+    c.sym_small = c.sym_split > 1;
+    unsigned char *base = nd->scratch;
+    c.xy = reinterpret_cast<double2 *>(base + kNoallocOffXy);
+    c.zm = reinterpret_cast<double2 *>(base + kNoallocOffZm);
+    c.hs = reinterpret_cast<double *>(base + kNoallocOffHs);
+    c.part = reinterpret_cast<double *>(base + kNoallocOffPart);
+    c.tile_hmax = reinterpret_cast<double *>(base + kNoallocOffHmax);
+    c.flags = reinterpret_cast<DevFlags *>(base + kNoallocOffFlags);
+    c.bad_h_sticky = reinterpret_cast<int *>(c.flags + 2);
+    c.cur_flags = c.flags;
+    c.kc.L = Lz;
+    c.kc.halfL = 0.5 * Lz;
+    {
+        uint64_t bits;
+        std::memcpy(&bits, &Lz, 8);
+        c.kc.L_hi = (int)(bits >> 32);
+        c.kc.L_lo = (int)(bits & 0xffffffffu);
+        const double hl = 0.5 * Lz;
+        std::memcpy(&bits, &hl, 8);
+        c.kc.halfL_hi = (int)(bits >> 32);
+    }
+    for (int k = 0; k <= MAX_NCUT_TABLE; ++k) {
+        const double kL = (double)k * Lz;
+        c.kc.c2nL[k] = 2.0 * kL;
+        c.kc.n2L2[k] = kL * kL;
+        c.kc.dn[k] = (double)k;
+    }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // the array keeps the previous call's contents: the flag blocks (max h, h <= 0) must start at zero
+    CK(cudaMemsetAsync(c.flags, 0, 3 * sizeof(DevFlags), s));
+    const ForceArgs f = {const_cast<double *>(x), const_cast<double *>(y), const_cast<double *>(z), m, h,
+                         gx, gy, gz, nullptr};
+    return enqueue_force_plain(ctx, f, 0u, false, s);
+}
+
 const char *steps_cyl_strerror(int code)
 {
     switch (code) {
@@ -1121,6 +1244,7 @@ const char *steps_cyl_strerror(int code)
     case STEPS_ESOFT: return "softening precondition violated (some h_i <= 0)";
     case STEPS_ECUDA: return "CUDA runtime error (see steps_cyl_last_cuda_error)";
     case STEPS_ENOMEM: return "out of memory";
+    case STEPS_ETOOBIG: return "n exceeds STEPS_CYL_NOALLOC_MAX_N, the fixed capacity of steps_cyl_accel_noalloc";
     case STEPS_EUNSUPPORTED: return "combination not built (EWALD_TABLE with the ORDERED_PAIRS flag, or a float table too large for shared memory)";
     default: return "unknown status";
     }
