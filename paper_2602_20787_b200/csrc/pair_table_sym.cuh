@@ -65,12 +65,17 @@ __device__ __forceinline__ void floor_frac(double x, int &i, double &f)
     f = x - (t - 4503599627370496.0);
 }
 
+// floor(x) and 1 + frac(x) as a float in [1, 2), for 0 <= x < 2^28, from ONE FP64 addition: x + 1.5 * 2^29 (rounded
+// down) lies in [2^29, 2^30), where a double's ulp is 2^-23, so its 52 mantissa bits are
+// [2^28 + floor(x) : 29 bits][frac(x) : 23 bits] -- the fraction truncated to 2^-23 of a cell, far below the float
+// nodes' own rounding.  A funnel shift and a mask give floor(x), one LOP3 the float.  (Any other x, NaN included,
+// gives SOME i in [0, 2^28) and SOME f1 in [1, 2): the callers clamp i from above and discard such lanes.)
 __device__ __forceinline__ void floor_frac1(double x, int &i, float &f1)
 {
-    const double t = __dadd_rd(x, 4503599627370496.0);            // 2^52 + floor(x), exact
-    i = lo32(t);
-    const double u = __dadd_rd(x, -(t - 4503599627370497.0));     // 1 + frac(x) in [1, 2)
-    f1 = __uint_as_float(0x3f800000u | (__funnelshift_l((unsigned)lo32(u), (unsigned)hi32(u), 3) & 0x007fffffu));
+    const double t = __dadd_rd(x, 805306368.0);                  // 1.5 * 2^29
+    const unsigned lo = (unsigned)lo32(t), hi = (unsigned)hi32(t);
+    i = (int)(__funnelshift_r(lo, hi, 23) & 0x0fffffffu);
+    f1 = __uint_as_float(0x3f800000u | (lo & 0x007fffffu));
 }
 
 template <class Tab>
@@ -174,9 +179,10 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Sha
         floor_frac1(az * tc.inv_dz, j0, fz1);
         const float fr = fr1 - 1.0f, fz = fz1 - 1.0f;
         // lanes beyond rho_max (and the padding particles) arrive here too: any node will do for them
-        // (j0 is in range for finite input; the clamp keeps a NaN coordinate from reading out of bounds)
-        i0 = min(max(i0, 0), tc.nrho - 1);
-        j0 = min(max(j0, 0), tc.nz - 1);
+        // (j0 is in range for finite input; the clamp keeps a NaN coordinate from reading out of bounds;
+        // floor_frac1 never returns a negative index)
+        i0 = min(i0, tc.nrho - 1);
+        j0 = min(j0, tc.nz - 1);
         // (this loop is bound by issue slots: redirecting the discarded lanes' gathers to one broadcast
         // address, as the TSC branch does, costs more in its SEL than it saves in bank conflicts)
         const float2 *d = D + (i0 + 1) * nzs + j0 + 1;
@@ -191,8 +197,8 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Sha
         floor_frac1(fma(rho, tc.inv_drho, 0.5), ic, fr1);
         floor_frac1(fma(az, tc.inv_dz, 0.5), jc, fz1);
         const float dr = fr1 - 1.5f, dz = fz1 - 1.5f;
-        ic = min(max(ic, 0), tc.nrho - 1);
-        jc = min(max(jc, 0), tc.nz - 1);
+        ic = min(ic, tc.nrho - 1);
+        jc = min(jc, tc.nz - 1);
         // node (ic - 1, jc - 1); lanes whose value is discarded all read node (-1, -1): one broadcast, no bank
         // conflicts (the nine gathers per pair make this loop shared-memory bound)
         const float2 *d = D + (live ? ic * nzs + jc : 0);
