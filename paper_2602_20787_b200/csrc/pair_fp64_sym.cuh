@@ -38,8 +38,11 @@
 namespace steps {
 
 #ifndef STEPS_SYM_UNROLL
-#define STEPS_SYM_UNROLL 1
+#define STEPS_SYM_UNROLL 2
 #endif
+// ring-loop unroll of every ring pass.  Measured at N = 1 048 576, N_cut = 5 (pair kernel, ms per evaluation):
+// 1 / 2 / 4 -> 3679.7 / 3640.4 / 3657.4.  (Unrolling ONLY the two-target main pass and leaving the single-target
+// passes of the diagonal tiles rolled measured 3700.0: the gain is in how ptxas schedules the whole kernel.)
 constexpr int kSymUnroll = STEPS_SYM_UNROLL;
 #ifndef STEPS_SYM_MINBLOCKS
 #define STEPS_SYM_MINBLOCKS 4      // resident CTAs per SM the register allocation aims at

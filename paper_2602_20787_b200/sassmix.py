@@ -11,7 +11,8 @@ Method.  `cuobjdump -sass` lists every kernel; in each pair kernel the loops are
 (`BRA` to a lower address).  The PAIR LOOP is the loop that reads a source from shared memory (`LDS`),
 contains no smaller loop that does, and holds the most arithmetic: one iteration of it evaluates
 `pairs_per_iteration` pair terms (symmetric kernels: two targets of a lane against one source, each
-result applied to both particles = 4 ordered interactions; ordered kernels: 1).  Instructions inside the
+result applied to both particles = 4 ordered interactions, times the ring steps an unrolled iteration holds -- read
+off its shuffle count; ordered kernels: 1).  Instructions inside the
 loop that a forward conditional branch can skip AND that lead to a CALL (the noinline spline of Eq. 3 behind
 its pre-test: the slow path) are tallied separately as `slowpath`; everything else is the mainline count.
 Kernels with a run-time image loop (template N_cut = 0) are marked `nested`: per_interaction() extrapolates
@@ -211,6 +212,10 @@ def tally(lib_path=LIB):
         inter = INTERACTIONS[fam]
         if fam == "pair_fp64_sym_kernel":        # <N_cut, FAR_ORDER2, target tiles per CTA>: 2 interactions per target
             inter = 2 * int(short.rstrip(">").split(",")[2])
+        if fam in ("pair_fp64_sym_kernel", "pair_fp64_round_kernel"):
+            # the ring loop may be unrolled (STEPS_SYM_UNROLL): one ring step moves the source's three double
+            # accumulators one lane down = 6 SHFL, so the shuffle count says how many steps an iteration holds
+            inter *= max(1, main.get("SHFL", 0) // 6)
         d = derive(main)
         kernels[short] = {
             "loop": ["0x%04x" % lo, "0x%04x" % hi], "interactions_per_iteration": inter, "nested": nested,
