@@ -65,9 +65,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
             os.unlink(SASSMIX)
         with open(stamp, "w") as f:
             f.write(want + "\n")
-    if not os.path.exists(SASSMIX):
-        # instruction tally of the pair loops of THIS binary (bench.py's roofline numerator)
-        from . import sassmix
+    # instruction tally of the pair loops of THIS binary (bench.py's roofline numerator): the file records the
+    # library's SHA-256, so a tally left behind by another build of the library is noticed and retaken
+    from . import sassmix
+    if not sassmix.is_current(LIB, SASSMIX):
         sassmix.write(LIB, SASSMIX)
     return LIB
 

@@ -194,6 +194,24 @@ def derive(kind_counts):
                 fp32_issue=fp32_issue, mufu=mufu, conv=conv, total=sum(v for k, v in c.items() if not k.startswith("fp64_t")))
 
 
+def file_sha256(path):
+    import hashlib
+    h = hashlib.sha256()
+    with open(path, "rb") as f:
+        for chunk in iter(lambda: f.read(1 << 20), b""):
+            h.update(chunk)
+    return h.hexdigest()
+
+
+def is_current(lib_path=LIB, out_path=None):
+    """True if the tally file beside `lib_path` was taken from exactly this binary."""
+    out_path = out_path or os.path.splitext(lib_path)[0] + ".sassmix.json"
+    try:
+        return load(out_path).get("library_sha256") == file_sha256(lib_path)
+    except (OSError, ValueError):
+        return False
+
+
 def tally(lib_path=LIB):
     sass = subprocess.run([_tool("cuobjdump"), "-sass", lib_path], check=True, capture_output=True,
                           text=True).stdout
@@ -225,7 +243,8 @@ def tally(lib_path=LIB):
             "variants": [{"loop": ["0x%04x" % l2, "0x%04x" % h2],
                           "per_interaction": {k: v / inter for k, v in derive(m2).items()}} for l2, h2, m2 in variants],
         }
-    return {"library": os.path.basename(lib_path), "tool": "cuobjdump -sass", "kernels": kernels}
+    return {"library": os.path.basename(lib_path), "library_sha256": file_sha256(lib_path), "tool": "cuobjdump -sass",
+            "kernels": kernels}
 
 
 def write(lib_path=LIB, out_path=None):

@@ -19,6 +19,7 @@ def mix():
     again = sassmix.tally(build.LIB)
     data = sassmix.load(build.SASSMIX)
     assert again["kernels"] == data["kernels"]
+    assert data["library_sha256"] == sassmix.file_sha256(build.LIB) and sassmix.is_current(build.LIB, build.SASSMIX)
     return data
 
 
