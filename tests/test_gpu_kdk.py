@@ -301,3 +301,47 @@ def test_accel_with_graph_flag(torch_cuda, oracle):
     with pytest.raises(b.StepsError):
         ctx.last_pair_kernel_ms()                 # the kernel is not timed on its own inside a graph
     ctx.close()
+
+
+def test_mixed_mode_kdk_across_a_reordering(torch_cuda, oracle):
+    """Mixed precision keeps its packed arrays in Morton order from N = 16 384 (order_kernels.cuh) and retakes the
+    order every 64 force evaluations; inputs and outputs stay in the CALLER's order.  70 KDK steps cross a
+    re-ordering: every particle must still be itself -- its trajectory agrees with the same steps taken in fp64
+    (caller-ordered arrays, no permutation) to mixed-precision accuracy, m and h are never written -- and the final
+    g must be the oracle's pair sum at the final positions on sampled targets (mixed bar: RMS 1e-5, max 1e-4)."""
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    torch = torch_cuda
+    w = workloads.make(1, n=16384, seed=43)
+    rng = np.random.default_rng(6)
+    v0 = [rng.normal(0, 0.05, w.n) for _ in range(3)]
+    dt, n_steps = 0.002, 70
+
+    def run(precision):
+        ctx = b.StepsCyl(n=w.n, Lz=w.Lz, G=w.G, n_cut=5, precision=precision)
+        dev = {k: _dev(torch, getattr(w, k)) for k in ("x", "y", "z", "m", "h")}
+        v = [_dev(torch, a) for a in v0]
+        g = [torch.empty(w.n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        ctx.accel(dev["x"], dev["y"], dev["z"], dev["m"], dev["h"], *g)
+        for _ in range(n_steps):
+            ctx.kdk_step(dev["x"], dev["y"], dev["z"], *v, dev["m"], dev["h"], *g, 1.0, 0.0, 1.0, 0.0, dt)
+        ctx.check()
+        stats = ctx.pass_stats()
+        ctx.close()
+        out = {k: t.cpu().numpy() for k, t in dev.items()}
+        return out, [t.cpu().numpy() for t in v], np.stack([t.cpu().numpy() for t in g], 1), stats
+
+    mx, mv, mg, (n_simple, n_pass) = run(b.PREC_MIXED)
+    dx, dv, dg, _ = run(b.PREC_FP64)
+    assert n_pass > 0 and 0 < n_simple <= n_pass            # the ordering is in use: some passes took the SIMPLE form
+    assert np.array_equal(mx["m"], w.m) and np.array_equal(mx["h"], w.h)
+    moved = np.hypot(dx["x"] - w.x, dx["y"] - w.y)
+    assert np.median(moved) > 1e-3                           # the particles did move ...
+    for k in ("x", "y"):                                     # ... and each one the way its fp64 twin did
+        assert np.abs(mx[k] - dx[k]).max() <= 1e-4 * max(1.0, moved.max())
+    for a, c in zip(mv, dv):
+        assert np.abs(a - c).max() <= 1e-4 * np.abs(c).max()
+    idx = workloads.sample_targets(w.n, 512, seed=9)
+    ref = np.stack(oracle.accel(mx["x"], mx["y"], mx["z"], w.m, w.h, w.Lz, w.G, 5, targets=idx), 1)
+    e = np.linalg.norm(mg[idx] - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert np.sqrt(np.mean(e ** 2)) <= 1e-5 and e.max() <= 1e-4, (np.sqrt(np.mean(e ** 2)), e.max())
