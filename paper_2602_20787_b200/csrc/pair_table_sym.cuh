@@ -20,6 +20,9 @@ namespace steps {
 
 struct TableConsts {
     const double2 *D;          // device table, nrho * nz nodes
+    const double2 *Dh;         // the same with a one-node halo on every side, (nrho + 2) * (nz + 2) nodes, the
+                               // boundary symmetries of D (reading T3) baked in: node (i, j), -1 <= i <= nrho,
+                               // -1 <= j <= nz, at Dh[(i + 1) * (nz + 2) + j + 1]  (TSC lookups in double)
     int nrho, nz, interp;
     double rho_max2;           // rho_max^2
     double inv_drho, inv_dz;   // 1 / node spacing
@@ -131,7 +134,9 @@ __device__ __forceinline__ double2 table_lookup(const TableConsts &tc, const Glo
         double rx = 0.0, ry = 0.0;
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const double2 v = table_node(tc, tab, ic - 1 + a, jc - 1 + b);
+            // the haloed table: no reflection, clamp or sign per node (9 sign multiplications and ~20 integer
+            // instructions less per lookup than table_node(); the values, hence the sums, are bit for bit the same)
+            const double2 v = __ldg(tc.Dh + (ic + a) * (tc.nz + 2) + jc + b);
             rx = fma(wz[b], v.x, rx);
             ry = fma(wz[b], v.y, ry);
         }

@@ -66,6 +66,7 @@ struct steps_cyl_ctx {
     GraphSlot gslot[2];                            // STEPS_FLAG_GRAPH: one captured evaluation per flag-block parity
     QuadNode *nodes = nullptr;
     double2 *d_table = nullptr;                    // EWALD_TABLE mode: D(rho, z), Eq. 17
+    double2 *d_table_halo = nullptr;               // the same with the symmetry halo (TableConsts::Dh)
     float2 *d_table_f32 = nullptr;                 // the same rounded to float (tab_fp32), staged in smem
     size_t table_smem_bytes = 0, table_mixed_smem_bytes = 0;
     TableConstsF32 tcf;
@@ -903,6 +904,27 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
                           pp.tab_rho_max, D.data());
         A(dev_alloc(&ctx->d_table, nodes));
         if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table, D.data(), nodes * sizeof(double2), cudaMemcpyHostToDevice));
+        {
+            // haloed copy for the double-precision TSC stencil: nodes outside the grid by the symmetries of D
+            // (D_rho odd in rho / even in z, D_z even in rho / odd in z about z = 0 and z = L/2; beyond the last
+            // radial node the last node) -- the rules of table_node() / stage_table_halo(), applied once here
+            const int nr = pp.tab_nrho, nzz = pp.tab_nz, nzs = nzz + 2;
+            std::vector<double> H((size_t)(nr + 2) * nzs * 2);
+            for (int i = -1; i <= nr; ++i)
+                for (int j = -1; j <= nzz; ++j) {
+                    int ii = i, jj = j;
+                    double sr = 1.0, sz = 1.0;
+                    if (ii < 0) { ii = -ii; sr = -1.0; }
+                    if (ii > nr - 1) ii = nr - 1;
+                    if (jj < 0) { jj = -jj; sz = -1.0; }
+                    if (jj > nzz - 1) { jj = 2 * (nzz - 1) - jj; sz = -sz; }
+                    const size_t src = ((size_t)ii * nzz + jj) * 2, dst = ((size_t)(i + 1) * nzs + (j + 1)) * 2;
+                    H[dst] = sr * D[src];
+                    H[dst + 1] = sz * D[src + 1];
+                }
+            A(dev_alloc(&ctx->d_table_halo, H.size() / 2));
+            if (rc == STEPS_OK) A(cudaMemcpy(ctx->d_table_halo, H.data(), H.size() * sizeof(double), cudaMemcpyHostToDevice));
+        }
         if (rc != STEPS_OK) return fail(rc);
         if (pp.tab_fp32) {
             // table rounded to float and staged in shared memory by a 512-thread CTA per SM
@@ -927,6 +949,7 @@ int steps_cyl_init(const steps_cyl_params *p, steps_cyl_ctx **out)
             if (rc != STEPS_OK) return fail(rc);
         }
         ctx->tc.D = ctx->d_table;
+        ctx->tc.Dh = ctx->d_table_halo;
         ctx->tc.nrho = pp.tab_nrho;
         ctx->tc.nz = pp.tab_nz;
         ctx->tc.interp = pp.interp;
@@ -973,7 +996,7 @@ void steps_cyl_destroy(steps_cyl_ctx *c)
         if (g.graph) cudaGraphDestroy(g.graph);
     }
     cudaFree(c->xy); cudaFree(c->zm); cudaFree(c->hs); cudaFree(c->tile_hmax); cudaFree(c->f_hi); cudaFree(c->f_lo);
-    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->perm); cudaFree(c->order_keys); cudaFree(c->rmax_bits); cudaFree(c->pass_stats); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_f32);
+    cudaFree(c->part); cudaFree(c->flags); cudaFree(c->perm); cudaFree(c->order_keys); cudaFree(c->rmax_bits); cudaFree(c->pass_stats); cudaFree(c->nodes); cudaFree(c->d_table); cudaFree(c->d_table_halo); cudaFree(c->d_table_f32);
     cudaFree(c->host_io); cudaFree(c->peak_out);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
