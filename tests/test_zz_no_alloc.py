@@ -102,3 +102,38 @@ def test_noalloc_matches_the_existing_path_on_calls_in_a_row(oracle):
     assert err.value.code == b.STEPS_ETOOBIG
     torch.cuda.synchronize()
     assert all(float(a.abs().max()) == 0.0 for a in t[5:])
+
+
+@pytest.mark.gpu
+def test_noalloc_can_be_captured_in_a_cuda_graph():
+    """What the entry point is for: after one ordinary call (the one-time set-up), a call under stream capture
+    records one memset and three kernels and nothing else; replaying the graph on new inputs written into the same
+    buffers gives what steps_cyl_accel gives for them."""
+    import torch
+    from paper_2602_20787_b200 import binding as b
+    from paper_2602_20787_b200 import workloads
+    assert torch.cuda.is_available(), "this test needs the B200; there is no CPU fallback"
+    wa = workloads.make(1, n=4000, seed=81)
+    wb = workloads.make(1, n=4000, seed=82)
+    n, L, G, nc = wa.n, wa.Lz, 1.0, 5
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (wa.x, wa.y, wa.z, wa.m, wa.h)]
+    out = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    b.accel_noalloc(n, L, G, nc, *ins, *out)                 # set-up happens here, outside capture
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        b.accel_noalloc(n, L, G, nc, *ins, *out)             # torch's current stream is the capturing stream
+    ctx = b.StepsCyl(n=n, Lz=L, G=G, n_cut=nc)
+    ref = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    for w in (wa, wb, wa):
+        for t, a in zip(ins, (w.x, w.y, w.z, w.m, w.h)):
+            t.copy_(torch.from_numpy(np.ascontiguousarray(a)))
+        for t in out:
+            t.fill_(float("nan"))
+        graph.replay()
+        ctx.accel(*ins, *ref)
+        ctx.check()
+        got = np.stack([t.cpu().numpy() for t in out], 1)
+        want = np.stack([t.cpu().numpy() for t in ref], 1)
+        assert np.all(np.isfinite(got)) and _rel(got, want).max() <= KERNEL_VS_KERNEL
+    ctx.close()
