@@ -319,29 +319,17 @@ __device__ __forceinline__ void image_sum_general(double rz, double rho2, double
                                                   int ncut, double &S, double &T)
 {
     const double hh2 = hh * hh;
+    int nlo = -ncut + 1, nhi = ncut - 1;
+    if (rz > 0.0) nhi = ncut;
+    if (rz < 0.0) nlo = -ncut;
     S = 0.0;
     T = 0.0;
-    // the images n = -N_cut+1 .. N_cut-1 are in every pair's window: a warp-uniform trip count and a double-valued
-    // counter (no I2F per image), so that the loop unrolls and the rsqrt chains of several images overlap -- this
-    // path is latency bound, not FP64 bound
-    double dn = (double)(1 - ncut);
-#pragma unroll 4
-    for (int c = 0; c < 2 * ncut - 1; ++c) {
-        const double d = fma(-dn, k.L, rz);
+    for (int n = nlo; n <= nhi; ++n) {
+        const double d = rz - (double)n * k.L;
         const double s2 = fma(d, d, rho2);
         const double w = (s2 < hh2) ? spline_w(s2, hh) : inv_cube_sqrt(s2);
         S += w;
-        T = fma(dn, w, T);
-        dn += 1.0;
-    }
-    // the end image n = sign(r_z) N_cut, absent when r_z == 0 (then |r_z - nL| = N_cut L is outside the strict window)
-    if (rz != 0.0) {
-        const double ne = copysign((double)ncut, rz);
-        const double d = fma(-ne, k.L, rz);
-        const double s2 = fma(d, d, rho2);
-        const double w = (s2 < hh2) ? spline_w(s2, hh) : inv_cube_sqrt(s2);
-        S += w;
-        T = fma(ne, w, T);
+        T = fma((double)n, w, T);
     }
 }
 
